@@ -1,0 +1,113 @@
+/* tslb.h -- C ABI of the B200-native TSLB + conservative Allen-Cahn hot path.
+ *
+ * Method: "Thread-safe multiphase lattice Boltzmann model for droplet and bubble dynamics at
+ * high density and viscosity contrasts", arXiv 2501.00846.  Citations "P:<line>" refer to the
+ * paper text and "Rk" to the readings listed in DESIGN.md.
+ *
+ * The library stores hydrodynamic moments, not populations: per lattice node the 14
+ * scalars p* (Eq. 11), u (Eq. 12), a2_neq (Eq. 13, 6 components), a = F/rho (Eq. 14-17, R5) and
+ * phi (Eq. 20), as structure-of-arrays planes, double buffered, x fastest:
+ *     idx = ix + nx * (iy + ny * iz).
+ * One tslb_step performs, for every node, the paper's four stages: interface
+ * tracking (Eq. 20), fused streaming-collision with recursive Hermite reconstruction
+ * (Eq. 7-10, 14), moments and forces (Eq. 11, 12, 3, 16, 17), pre-regularisation (Eq. 13).
+ *
+ * Everything runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.  All
+ * functions are thread-compatible (one handle per thread at a time) and enqueue work on the
+ * handle's stream without synchronising; the caller synchronises the stream.
+ *
+ * Errors: 0 on success, negative otherwise; tslb_last_error() returns a thread-local text.
+ *   TSLB_EINVAL   (-1) bad argument (non-positive size, n < 0, NULL, non-positive rho/mu/
+ *                      delta/mobility, sigma < 0, unknown enum, axis shorter than the stencil)
+ *   TSLB_EWORKSPACE(-2) workspace NULL, too small or not 256-byte aligned
+ *   TSLB_ECUDA    (-3) a CUDA call failed (text holds cudaGetErrorString)
+ *   TSLB_ESTATE   (-4) tslb_step / tslb_get before tslb_init
+ */
+#ifndef TSLB_H
+#define TSLB_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tslb_handle tslb_handle; /* opaque; host memory owned by the library */
+
+enum { TSLB_BC_PERIODIC = 0, TSLB_BC_WALL = 1 }; /* per axis, both ends */
+enum { TSLB_F32 = 0, TSLB_F64 = 1 };
+enum { TSLB_OK = 0, TSLB_EINVAL = -1, TSLB_EWORKSPACE = -2, TSLB_ECUDA = -3, TSLB_ESTATE = -4 };
+
+/* flags (bit field) */
+enum {
+  TSLB_FLAG_NAIVE = 1 /* run the one-thread-per-node global-memory kernels (debug/validation
+                         path, same arithmetic contract); default 0 = tiled z-marching kernels */
+};
+
+typedef struct tslb_params {
+  double rho_l, rho_g;   /* > 0 ; rho = rho_g + phi (rho_l - rho_g)      */
+  double mu_l, mu_g;     /* > 0 ; dynamic viscosities, mixed linearly in phi (R14) */
+  double sigma;          /* >= 0 ; beta = 12 sigma/delta, kappa_mu = 3 sigma delta/2 P:136     */
+  double delta;          /* > 0 ; interface width in lattice units */
+  double mobility;       /* > 0 ; D of Eq. 4 ; kappa_AC = 4 D/delta    */
+  double body_accel[3];  /* g ; force density (rho - rho_l) g : light phase only    P:256, R20 */
+  int bc[3];             /* TSLB_BC_* for x, y, z                                              */
+  int precision;         /* TSLB_F32 / TSLB_F64 : type of every field pointer and of all math  */
+  int flags;             /* TSLB_FLAG_* ; 0 for the production path                            */
+} tslb_params;
+
+/* Bytes of device workspace tslb_create needs for this size and precision (0 on bad input). */
+size_t tslb_workspace_bytes(int nx, int ny, int nz, const tslb_params *params);
+
+/* Create a solver on the CALLER-OWNED device buffer `workspace` (>= tslb_workspace_bytes,
+ * 256-byte aligned, kept alive until tslb_destroy).  The library carves its double-buffered SoA
+ * planes out of it and allocates nothing else on the device.  `stream` is a cudaStream_t (NULL =
+ * legacy default stream).  Minimum size: 4 nodes on a periodic axis, 2 on a wall axis.  No
+ * kernel is launched. */
+int tslb_create(int nx, int ny, int nz, const tslb_params *params, void *workspace, void *stream,
+                tslb_handle **out);
+
+/* Set the initial state from DEVICE arrays in the handle's precision: phi[N], u[3][N] (three
+ * consecutive planes ux, uy, uz).  p* = 0 and a2_neq = 0 (R9); a = (F^s + F^b)/rho from phi with
+ * the same ghost rules as the step (R19).  The arrays are not retained.  May be called again. */
+int tslb_init(tslb_handle *h, const void *phi, const void *u);
+
+/* Advance n >= 0 time steps (n = 0 is a no-op).  No host synchronisation inside. */
+int tslb_step(tslb_handle *h, int n);
+
+/* Write rho = rho_g + clamp(phi)(rho_l - rho_g) (R15), p = p* rho cs^2, the
+ * velocity u of Eq. 12 ([3][N]) and phi into DEVICE arrays of the handle's precision.  A NULL
+ * pointer skips that field. */
+int tslb_get(tslb_handle *h, void *rho, void *p, void *u, void *phi);
+
+/* Full internal state (debug / parity of the unexposed fields): p*[N], u[3][N], a2_neq[6][N] in
+ * the order xx,yy,zz,xy,xz,yz, a[3][N], phi[N]; DEVICE arrays, NULL skips. */
+int tslb_get_state(tslb_handle *h, void *pstar, void *u, void *A, void *a, void *phi);
+
+/* Host-buffer convenience for end-to-end use: same as tslb_init / tslb_get but the field
+ * pointers are HOST arrays (pinned memory makes the copies asynchronous); the library stages
+ * them through the spare state buffer, so no extra device memory is needed.  tslb_get_host
+ * synchronises the stream before returning. */
+int tslb_init_host(tslb_handle *h, const void *phi, const void *u);
+int tslb_get_host(tslb_handle *h, void *rho, void *p, void *u, void *phi);
+
+/* Same as tslb_step, but brackets every kernel with CUDA events on the handle's stream,
+ * synchronises, and ADDS the elapsed milliseconds per kernel kind into kernel_ms[TSLB_NKERNELS]
+ * (caller-zeroed HOST array).  Used by bench.py for the per-kernel roofline. */
+enum { TSLB_K_NORMAL = 0,          /* naive path only: sharpening-flux kernel            */
+       TSLB_K_ALLEN_CAHN = 1,      /* interface tracking, Eq. 20                          */
+       TSLB_K_STREAM_COLLIDE = 2,  /* fused stream-collide-moments-forces, Eq. 7-17       */
+       TSLB_NKERNELS = 4 };
+int tslb_step_timed(tslb_handle *h, int n, float *kernel_ms);
+
+/* Number of kernel launches the handle has enqueued so far (for bench.py's gpu_launches). */
+long long tslb_launch_count(const tslb_handle *h);
+
+void tslb_destroy(tslb_handle *h); /* frees host memory only; NULL is allowed */
+
+const char *tslb_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TSLB_H */

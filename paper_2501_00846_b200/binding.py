@@ -1,0 +1,205 @@
+"""Thin Python binding of the C ABI in include/tslb.h (same names, argument marshalling only).
+
+PyTorch supplies device memory and streams; every step of the path runs in the CUDA kernels of
+libtslb.so.  There is no CPU fallback: a missing library or a missing GPU raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtslb.so")
+
+BC_PERIODIC, BC_WALL = 0, 1
+F32, F64 = 0, 1
+FLAG_NAIVE = 1
+
+SYMBOLS = ("tslb_workspace_bytes", "tslb_create", "tslb_init", "tslb_step", "tslb_get",
+           "tslb_get_state", "tslb_init_host", "tslb_get_host", "tslb_step_timed",
+           "tslb_launch_count",
+           "tslb_destroy", "tslb_last_error")
+
+
+class tslb_params(C.Structure):
+    _fields_ = [("rho_l", C.c_double), ("rho_g", C.c_double),
+                ("mu_l", C.c_double), ("mu_g", C.c_double),
+                ("sigma", C.c_double), ("delta", C.c_double), ("mobility", C.c_double),
+                ("body_accel", C.c_double * 3), ("bc", C.c_int * 3),
+                ("precision", C.c_int), ("flags", C.c_int)]
+
+
+def make_params(rho_l, rho_g, mu_l, mu_g, sigma, delta, mobility, body_accel=(0.0, 0.0, 0.0),
+                bc=(0, 0, 0), precision=F64, flags=0):
+    p = tslb_params()
+    p.rho_l, p.rho_g, p.mu_l, p.mu_g = rho_l, rho_g, mu_l, mu_g
+    p.sigma, p.delta, p.mobility = sigma, delta, mobility
+    p.body_accel[:] = [float(v) for v in body_accel]
+    p.bc[:] = [int(v) for v in bc]
+    p.precision, p.flags = int(precision), int(flags)
+    return p
+
+
+_lib = None
+
+
+def load():
+    """dlopen libtslb.so and declare the prototypes.  Raises if the library is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run __graft_entry__.build() "
+                           "(python -m paper_2501_00846_b200.build); there is no CPU fallback")
+    lib = C.CDLL(LIB_PATH)
+    vp = C.c_void_p
+    lib.tslb_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(tslb_params)]
+    lib.tslb_workspace_bytes.restype = C.c_size_t
+    lib.tslb_create.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(tslb_params), vp, vp,
+                                C.POINTER(vp)]
+    lib.tslb_init.argtypes = [vp, vp, vp]
+    lib.tslb_step.argtypes = [vp, C.c_int]
+    lib.tslb_get.argtypes = [vp, vp, vp, vp, vp]
+    lib.tslb_get_state.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.tslb_init_host.argtypes = [vp, vp, vp]
+    lib.tslb_get_host.argtypes = [vp, vp, vp, vp, vp]
+    lib.tslb_step_timed.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
+    lib.tslb_launch_count.argtypes = [vp]
+    lib.tslb_launch_count.restype = C.c_longlong
+    lib.tslb_destroy.argtypes = [vp]
+    lib.tslb_destroy.restype = None
+    lib.tslb_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+class TslbError(RuntimeError):
+    pass
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise TslbError(f"{what} failed ({rc}): {load().tslb_last_error().decode()}")
+
+
+def tslb_workspace_bytes(nx, ny, nz, params):
+    return int(load().tslb_workspace_bytes(nx, ny, nz, C.byref(params)))
+
+
+class Solver:
+    """tslb_create / tslb_init / tslb_step / tslb_get on torch device memory.
+
+    Fields are torch tensors shaped (nz, ny, nx) (x fastest), vectors (3, nz, ny, nx), in the
+    solver's precision, on the solver's device.  The workspace tensor is owned here."""
+
+    def __init__(self, nx, ny, nz, params, precision="f64", flags=0, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("tslb needs a CUDA device (no CPU fallback)")
+        self.torch = torch
+        self.lib = load()
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.shape = (self.nz, self.ny, self.nx)
+        self.device = torch.device(device)
+        self.dtype = torch.float64 if precision == "f64" else torch.float32
+        self.np_dtype = np.float64 if precision == "f64" else np.float32
+        prm = dict(params)
+        prm["precision"] = F64 if precision == "f64" else F32
+        prm["flags"] = flags
+        self.params = make_params(**prm)
+        nbytes = tslb_workspace_bytes(nx, ny, nz, self.params)
+        if nbytes == 0:
+            raise TslbError("tslb_workspace_bytes: bad size or parameters")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        assert self.workspace.data_ptr() % 256 == 0
+        self._h = C.c_void_p()
+        _check(self.lib.tslb_create(nx, ny, nz, C.byref(self.params), self.workspace.data_ptr(),
+                                    self.stream.cuda_stream, C.byref(self._h)), "tslb_create")
+
+    # -- helpers -------------------------------------------------------------------------
+    def _dev(self, a, shape):
+        t = self.torch.as_tensor(a)
+        t = t.to(device=self.device, dtype=self.dtype).contiguous()
+        assert tuple(t.shape) == shape, (tuple(t.shape), shape)
+        return t
+
+    def _empty(self, *lead):
+        return self.torch.empty(tuple(lead) + self.shape, dtype=self.dtype, device=self.device)
+
+    # -- the ABI calls -------------------------------------------------------------------
+    def init(self, phi, u):
+        """tslb_init from device tensors (host arrays are copied to the device by torch first)."""
+        phi = self._dev(phi, self.shape)
+        u = self._dev(u, (3,) + self.shape)
+        with self.torch.cuda.stream(self.stream):
+            _check(self.lib.tslb_init(self._h, phi.data_ptr(), u.data_ptr()), "tslb_init")
+        self.stream.synchronize()          # phi, u may be temporaries
+
+    def init_host(self, phi, u):
+        """tslb_init_host from host arrays/tensors of the solver's precision (pinned = async)."""
+        phi, u = self._host_ptr(phi, self.shape), self._host_ptr(u, (3,) + self.shape)
+        _check(self.lib.tslb_init_host(self._h, phi[1], u[1]), "tslb_init_host")
+        self.stream.synchronize()
+        return self
+
+    def step(self, n=1):
+        _check(self.lib.tslb_step(self._h, int(n)), "tslb_step")
+
+    def step_timed(self, n=1):
+        """tslb_step_timed: returns {kernel kind: total ms over the n steps} (synchronises)."""
+        ms = (C.c_float * 4)()
+        _check(self.lib.tslb_step_timed(self._h, int(n), ms), "tslb_step_timed")
+        names = ("normal", "allen_cahn", "stream_collide", "reserved")
+        return {k: float(v) for k, v in zip(names, ms) if v > 0.0}
+
+    def get(self, want=("rho", "p", "u", "phi")):
+        out = {k: (self._empty(3) if k == "u" else self._empty()) for k in want}
+        ptr = lambda k: out[k].data_ptr() if k in out else None
+        _check(self.lib.tslb_get(self._h, ptr("rho"), ptr("p"), ptr("u"), ptr("phi")), "tslb_get")
+        return out
+
+    def get_state(self):
+        out = dict(pstar=self._empty(), u=self._empty(3), A=self._empty(6), a=self._empty(3),
+                   phi=self._empty())
+        _check(self.lib.tslb_get_state(self._h, out["pstar"].data_ptr(), out["u"].data_ptr(),
+                                       out["A"].data_ptr(), out["a"].data_ptr(),
+                                       out["phi"].data_ptr()), "tslb_get_state")
+        return out
+
+    def get_host(self, out):
+        """tslb_get_host into a dict of host arrays/tensors {rho,p,u,phi} (any subset)."""
+        ptrs = {k: self._host_ptr(v, ((3,) if k == "u" else ()) + self.shape)[1]
+                for k, v in out.items()}
+        _check(self.lib.tslb_get_host(self._h, ptrs.get("rho"), ptrs.get("p"), ptrs.get("u"),
+                                      ptrs.get("phi")), "tslb_get_host")
+        return out
+
+    def _host_ptr(self, a, shape):
+        if isinstance(a, np.ndarray):
+            assert a.dtype == self.np_dtype and a.flags.c_contiguous and a.shape == shape
+            return a, a.ctypes.data
+        assert a.device.type == "cpu" and a.dtype == self.dtype and a.is_contiguous()
+        assert tuple(a.shape) == shape
+        return a, a.data_ptr()
+
+    @property
+    def launches(self):
+        return int(self.lib.tslb_launch_count(self._h))
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.stream.synchronize()
+            self.lib.tslb_destroy(self._h)
+            self._h = C.c_void_p()
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

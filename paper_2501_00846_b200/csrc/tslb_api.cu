@@ -1,0 +1,293 @@
+// tslb_api.cu -- the C ABI of include/tslb.h: argument checking, workspace carving, launches.
+// Every step of the path runs in the kernels of tslb_tiled.cuh / tslb_naive.cuh.
+#include "../../include/tslb.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "tslb_device.cuh"
+#include "tslb_naive.cuh"
+#include "tslb_tiled.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, const char* a = "", const char* b = "") {
+  snprintf(g_err, sizeof(g_err), fmt, a, b);
+  return code;
+}
+
+#define CUDA_TRY(call)                                                                   \
+  do {                                                                                   \
+    cudaError_t e__ = (call);                                                            \
+    if (e__ != cudaSuccess) return fail(TSLB_ECUDA, "%s: %s", #call, cudaGetErrorString(e__)); \
+  } while (0)
+
+constexpr size_t kAlign = 256;
+size_t round_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+bool params_ok(int nx, int ny, int nz, const tslb_params* p) {
+  if (!p || nx < 1 || ny < 1 || nz < 1) return false;
+  if (!(p->rho_l > 0 && p->rho_g > 0 && p->mu_l > 0 && p->mu_g > 0 && p->delta > 0 &&
+        p->mobility > 0 && p->sigma >= 0))
+    return false;
+  if (p->precision != TSLB_F32 && p->precision != TSLB_F64) return false;
+  if (p->flags & ~TSLB_FLAG_NAIVE) return false;
+  const int n[3] = {nx, ny, nz};
+  for (int d = 0; d < 3; ++d) {
+    if (p->bc[d] != TSLB_BC_PERIODIC && p->bc[d] != TSLB_BC_WALL) return false;
+    if (n[d] < (p->bc[d] == TSLB_BC_PERIODIC ? 4 : 2)) return false;
+  }
+  if ((long long)nx * ny * nz > (1LL << 31) - 1) return false;   // 32-bit in-plane indexing
+  return true;
+}
+
+size_t elem_size(const tslb_params* p) { return p->precision == TSLB_F64 ? 8 : 4; }
+// bytes of one SoA plane, padded so that every plane starts 256-byte aligned
+size_t plane_bytes(long long N, size_t es) { return round_up(size_t(N) * es); }
+int scratch_planes(const tslb_params* p) { return (p->flags & TSLB_FLAG_NAIVE) ? 3 : 0; }
+
+template <typename T>
+tslb::DevParams<T> make_dev(int nx, int ny, int nz, const tslb_params& p, long long stride) {
+  tslb::DevParams<T> d;
+  d.nx = nx; d.ny = ny; d.nz = nz;
+  d.bcx = p.bc[0]; d.bcy = p.bc[1]; d.bcz = p.bc[2];
+  d.N = stride;
+  d.rho_l = T(p.rho_l); d.rho_g = T(p.rho_g); d.drho = T(p.rho_l - p.rho_g);
+  d.mu_g = T(p.mu_g); d.dmu = T(p.mu_l - p.mu_g);
+  d.beta4 = T(4.0 * 12.0 * p.sigma / p.delta);
+  d.kappa_mu = T(3.0 * p.sigma * p.delta / 2.0);
+  d.mob = T(p.mobility);
+  d.kappa_ac = T(4.0 * p.mobility / p.delta);
+  d.gx = T(p.body_accel[0]); d.gy = T(p.body_accel[1]); d.gz = T(p.body_accel[2]);
+  return d;
+}
+
+}  // namespace
+
+struct tslb_handle {
+  int nx, ny, nz;
+  long long nodes;       // nx ny nz
+  long long stride;      // elements between consecutive SoA planes (>= nodes, plane 256-B aligned)
+  tslb_params prm;
+  size_t es;
+  cudaStream_t stream;
+  char* buf[2];          // two state buffers of NFIELD planes
+  char* scratch;         // naive path only: 3 planes
+  int cur;
+  bool inited;
+  long long launches;
+};
+
+extern "C" {
+
+const char* tslb_last_error(void) { return g_err; }
+
+size_t tslb_workspace_bytes(int nx, int ny, int nz, const tslb_params* p) {
+  if (!params_ok(nx, ny, nz, p)) return 0;
+  size_t pb = plane_bytes((long long)nx * ny * nz, elem_size(p));
+  return pb * size_t(2 * tslb::NFIELD + scratch_planes(p));
+}
+
+int tslb_create(int nx, int ny, int nz, const tslb_params* p, void* workspace, void* stream,
+                tslb_handle** out) {
+  if (!out) return fail(TSLB_EINVAL, "tslb_create: out is NULL");
+  *out = nullptr;
+  if (!params_ok(nx, ny, nz, p)) return fail(TSLB_EINVAL, "tslb_create: bad size or parameters");
+  if (!workspace || (reinterpret_cast<size_t>(workspace) % kAlign) != 0)
+    return fail(TSLB_EWORKSPACE, "tslb_create: workspace NULL or not 256-byte aligned");
+  tslb_handle* h = new (std::nothrow) tslb_handle();
+  if (!h) return fail(TSLB_EINVAL, "tslb_create: out of host memory");
+  h->nx = nx; h->ny = ny; h->nz = nz;
+  h->nodes = (long long)nx * ny * nz;
+  h->prm = *p;
+  h->es = elem_size(p);
+  size_t pb = plane_bytes(h->nodes, h->es);
+  h->stride = (long long)(pb / h->es);
+  h->stream = static_cast<cudaStream_t>(stream);
+  char* w = static_cast<char*>(workspace);
+  h->buf[0] = w;
+  h->buf[1] = w + pb * tslb::NFIELD;
+  h->scratch = scratch_planes(p) ? w + pb * 2 * tslb::NFIELD : nullptr;
+  h->cur = 0;
+  h->inited = false;
+  h->launches = 0;
+  *out = h;
+  return TSLB_OK;
+}
+
+void tslb_destroy(tslb_handle* h) { delete h; }
+
+long long tslb_launch_count(const tslb_handle* h) { return h ? h->launches : 0; }
+
+}  // extern "C"
+
+// ------------------------------------------------------------------ typed implementations
+namespace {
+
+template <typename T>
+int init_impl(tslb_handle* h, const T* phi, const T* u, long long u_stride) {
+  auto P = make_dev<T>(h->nx, h->ny, h->nz, h->prm, h->stride);
+  T* D = reinterpret_cast<T*>(h->buf[0]);
+  h->cur = 0;
+  unsigned blocks = unsigned((h->nodes + 255) / 256);
+  tslb::k_init<T><<<blocks, 256, 0, h->stream>>>(P, h->nodes, phi, u, u_stride, D);
+  h->launches += 1;
+  CUDA_TRY(cudaGetLastError());
+  h->inited = true;
+  return TSLB_OK;
+}
+
+template <typename T>
+int step_impl(tslb_handle* h, int n, const tslb::Marker& mk) {
+  auto P = make_dev<T>(h->nx, h->ny, h->nz, h->prm, h->stride);
+  for (int it = 0; it < n; ++it) {
+    const T* S = reinterpret_cast<const T*>(h->buf[h->cur]);
+    T* D = reinterpret_cast<T*>(h->buf[h->cur ^ 1]);
+    if (h->prm.flags & TSLB_FLAG_NAIVE) {
+      T* Q = reinterpret_cast<T*>(h->scratch);
+      unsigned b256 = unsigned((h->nodes + 255) / 256), b128 = unsigned((h->nodes + 127) / 128);
+      tslb::k_normal_naive<T><<<b256, 256, 0, h->stream>>>(P, h->nodes, S, Q);
+      mk.mark(TSLB_K_NORMAL);
+      tslb::k_allen_cahn_naive<T><<<b256, 256, 0, h->stream>>>(P, h->nodes, S, Q,
+                                                               D + tslb::F_PHI * P.N);
+      mk.mark(TSLB_K_ALLEN_CAHN);
+      tslb::k_stream_collide_naive<T><<<b128, 128, 0, h->stream>>>(P, h->nodes, S, D);
+      mk.mark(TSLB_K_STREAM_COLLIDE);
+      h->launches += 3;
+    } else {
+      int rc = tslb::launch_step_tiled<T>(P, S, D, h->stream, &h->launches, mk);
+      if (rc != 0) return fail(TSLB_ECUDA, "tiled launch: %s", cudaGetErrorString(cudaError_t(rc)));
+    }
+    h->cur ^= 1;
+  }
+  CUDA_TRY(cudaGetLastError());
+  return TSLB_OK;
+}
+
+template <typename T>
+int get_impl(tslb_handle* h, T* rho, T* p, T* u, long long u_stride, T* phi) {
+  auto P = make_dev<T>(h->nx, h->ny, h->nz, h->prm, h->stride);
+  const T* S = reinterpret_cast<const T*>(h->buf[h->cur]);
+  unsigned blocks = unsigned((h->nodes + 255) / 256);
+  tslb::k_get<T><<<blocks, 256, 0, h->stream>>>(P, h->nodes, S, rho, p, u, u_stride, phi);
+  h->launches += 1;
+  CUDA_TRY(cudaGetLastError());
+  return TSLB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tslb_init(tslb_handle* h, const void* phi, const void* u) {
+  if (!h || !phi || !u) return fail(TSLB_EINVAL, "tslb_init: NULL argument");
+  if (h->prm.precision == TSLB_F64)
+    return init_impl<double>(h, static_cast<const double*>(phi), static_cast<const double*>(u),
+                             h->nodes);
+  return init_impl<float>(h, static_cast<const float*>(phi), static_cast<const float*>(u),
+                          h->nodes);
+}
+
+int tslb_step(tslb_handle* h, int n) {
+  if (!h || n < 0) return fail(TSLB_EINVAL, "tslb_step: NULL handle or n < 0");
+  if (!h->inited) return fail(TSLB_ESTATE, "tslb_step before tslb_init");
+  tslb::Marker none;
+  return h->prm.precision == TSLB_F64 ? step_impl<double>(h, n, none)
+                                      : step_impl<float>(h, n, none);
+}
+
+int tslb_step_timed(tslb_handle* h, int n, float* kernel_ms) {
+  if (!h || n < 0 || !kernel_ms) return fail(TSLB_EINVAL, "tslb_step_timed: bad argument");
+  if (!h->inited) return fail(TSLB_ESTATE, "tslb_step_timed before tslb_init");
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> kind;
+  tslb::Marker mk;
+  mk.events = &ev; mk.kinds = &kind; mk.stream = h->stream;
+  mk.mark(-1);
+  int rc = h->prm.precision == TSLB_F64 ? step_impl<double>(h, n, mk) : step_impl<float>(h, n, mk);
+  cudaError_t e = cudaStreamSynchronize(h->stream);
+  for (size_t i = 1; i < ev.size() && e == cudaSuccess; ++i) {
+    float ms = 0.f;
+    e = cudaEventElapsedTime(&ms, ev[i - 1], ev[i]);
+    if (kind[i] >= 0 && kind[i] < TSLB_NKERNELS) kernel_ms[kind[i]] += ms;
+  }
+  for (cudaEvent_t x : ev) cudaEventDestroy(x);
+  if (rc != TSLB_OK) return rc;
+  if (e != cudaSuccess) return fail(TSLB_ECUDA, "tslb_step_timed: %s", cudaGetErrorString(e));
+  return TSLB_OK;
+}
+
+int tslb_get(tslb_handle* h, void* rho, void* p, void* u, void* phi) {
+  if (!h) return fail(TSLB_EINVAL, "tslb_get: NULL handle");
+  if (!h->inited) return fail(TSLB_ESTATE, "tslb_get before tslb_init");
+  if (h->prm.precision == TSLB_F64)
+    return get_impl<double>(h, (double*)rho, (double*)p, (double*)u, h->nodes, (double*)phi);
+  return get_impl<float>(h, (float*)rho, (float*)p, (float*)u, h->nodes, (float*)phi);
+}
+
+int tslb_get_state(tslb_handle* h, void* pstar, void* u, void* A, void* a, void* phi) {
+  if (!h) return fail(TSLB_EINVAL, "tslb_get_state: NULL handle");
+  if (!h->inited) return fail(TSLB_ESTATE, "tslb_get_state before tslb_init");
+  const char* S = h->buf[h->cur];
+  const size_t pb = size_t(h->stride) * h->es, nb = size_t(h->nodes) * h->es;
+  struct { void* dst; int first, count; } parts[5] = {
+      {pstar, tslb::F_P, 1}, {u, tslb::F_UX, 3}, {A, tslb::F_AXX, 6}, {a, tslb::F_AX, 3},
+      {phi, tslb::F_PHI, 1}};
+  for (auto& q : parts) {
+    if (!q.dst) continue;
+    for (int k = 0; k < q.count; ++k)
+      CUDA_TRY(cudaMemcpyAsync(static_cast<char*>(q.dst) + nb * k, S + pb * (q.first + k), nb,
+                               cudaMemcpyDeviceToDevice, h->stream));
+  }
+  return TSLB_OK;
+}
+
+int tslb_init_host(tslb_handle* h, const void* phi, const void* u) {
+  if (!h || !phi || !u) return fail(TSLB_EINVAL, "tslb_init_host: NULL argument");
+  // stage phi, u in planes 0..3 of the second buffer, then run the init kernel into buffer 0
+  char* stage = h->buf[1];
+  const size_t pb = size_t(h->stride) * h->es, nb = size_t(h->nodes) * h->es;
+  CUDA_TRY(cudaMemcpyAsync(stage, phi, nb, cudaMemcpyHostToDevice, h->stream));
+  for (int k = 0; k < 3; ++k)
+    CUDA_TRY(cudaMemcpyAsync(stage + pb * (1 + k), static_cast<const char*>(u) + nb * k, nb,
+                             cudaMemcpyHostToDevice, h->stream));
+  if (h->prm.precision == TSLB_F64)
+    return init_impl<double>(h, (const double*)stage, (const double*)(stage + pb), h->stride);
+  return init_impl<float>(h, (const float*)stage, (const float*)(stage + pb), h->stride);
+}
+
+int tslb_get_host(tslb_handle* h, void* rho, void* p, void* u, void* phi) {
+  if (!h) return fail(TSLB_EINVAL, "tslb_get_host: NULL handle");
+  if (!h->inited) return fail(TSLB_ESTATE, "tslb_get_host before tslb_init");
+  // derived fields go to planes 0..5 of the spare buffer, then to the host
+  char* stage = h->buf[h->cur ^ 1];
+  const size_t pb = size_t(h->stride) * h->es, nb = size_t(h->nodes) * h->es;
+  void* d_rho = rho ? stage : nullptr;
+  void* d_p = p ? stage + pb : nullptr;
+  void* d_u = u ? stage + 2 * pb : nullptr;
+  void* d_phi = phi ? stage + 5 * pb : nullptr;
+  int rc;
+  if (h->prm.precision == TSLB_F64)
+    rc = get_impl<double>(h, (double*)d_rho, (double*)d_p, (double*)d_u, h->stride, (double*)d_phi);
+  else
+    rc = get_impl<float>(h, (float*)d_rho, (float*)d_p, (float*)d_u, h->stride, (float*)d_phi);
+  if (rc != TSLB_OK) return rc;
+  if (rho) CUDA_TRY(cudaMemcpyAsync(rho, d_rho, nb, cudaMemcpyDeviceToHost, h->stream));
+  if (p) CUDA_TRY(cudaMemcpyAsync(p, d_p, nb, cudaMemcpyDeviceToHost, h->stream));
+  if (u)
+    for (int k = 0; k < 3; ++k)
+      CUDA_TRY(cudaMemcpyAsync(static_cast<char*>(u) + nb * k, static_cast<char*>(d_u) + pb * k, nb,
+                               cudaMemcpyDeviceToHost, h->stream));
+  if (phi) CUDA_TRY(cudaMemcpyAsync(phi, d_phi, nb, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return TSLB_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,223 @@
+// tslb_naive.cuh -- one-thread-per-node global-memory kernels (TSLB_FLAG_NAIVE).
+//
+// Validation path: same arithmetic contract as the tiled kernels, no shared memory, every
+// neighbour value fetched through L1/L2.  Also hosts the init and get kernels, which are not on
+// the per-step path.
+#pragma once
+#include "tslb_device.cuh"
+
+namespace tslb {
+
+template <typename T>
+__device__ __forceinline__ void node_coords(const DevParams<T>& P, long long idx, int& ix, int& iy,
+                                            int& iz) {
+  ix = int(idx % P.nx);
+  long long r = idx / P.nx;
+  iy = int(r % P.ny);
+  iz = int(r / P.ny);
+}
+
+// Neighbour at offset (dx,dy,dz), |d| <= 2: linear index and per-axis wall-crossing flags.
+template <typename T>
+__device__ __forceinline__ long long nbr(const DevParams<T>& P, int ix, int iy, int iz, int dx,
+                                         int dy, int dz, int& kx, int& ky, int& kz) {
+  int jx = ghost_index(ix + dx, P.nx, P.bcx, kx);
+  int jy = ghost_index(iy + dy, P.ny, P.bcy, ky);
+  int jz = ghost_index(iz + dz, P.nz, P.bcz, kz);
+  return jx + (long long)P.nx * (jy + (long long)P.ny * jz);
+}
+
+// Isotropic gradient (Eq. 18) and Laplacian (Eq. 19 as repaired by R10) of a scalar plane.
+template <typename T>
+__device__ __forceinline__ void grad_lap(const DevParams<T>& P, const T* __restrict__ phi, int ix,
+                                         int iy, int iz, T& gx, T& gy, T& gz, T& lap) {
+  T sx = 0, sy = 0, sz = 0, sw = 0;
+#pragma unroll
+  for (int i = 0; i < 27; ++i) {
+    const int cx = i % 3 - 1, cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
+    int kx, ky, kz;
+    T v = phi[nbr(P, ix, iy, iz, cx, cy, cz, kx, ky, kz)];
+    T w = w1<T>(cx) * w1<T>(cy) * w1<T>(cz);
+    sw = fma(w, v, sw);
+    if (cx) sx = fma(w * T(cx), v, sx);
+    if (cy) sy = fma(w * T(cy), v, sy);
+    if (cz) sz = fma(w * T(cz), v, sz);
+  }
+  gx = T(3) * sx; gy = T(3) * sy; gz = T(3) * sz;
+  // (2/cs^2) sum_{i!=0} w_i (phi_i - phi_0) = 6 (sum_i w_i phi_i - phi_0)
+  lap = T(6) * (sw - phi[ix + (long long)P.nx * (iy + (long long)P.ny * iz)]);
+}
+
+// ---- stage K4a: sharpening flux  Qs = phi (1 - phi) grad(phi)/sqrt(|grad(phi)|^2 + eps^2)  (R13)
+template <typename T>
+__global__ void __launch_bounds__(256) k_normal_naive(DevParams<T> P, long long nodes,
+                                                      const T* __restrict__ S,
+                                                      T* __restrict__ Q) {
+  long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= nodes) return;
+  int ix, iy, iz;
+  node_coords(P, idx, ix, iy, iz);
+  const T* phi = S + F_PHI * P.N;
+  T gx, gy, gz, lap;
+  grad_lap(P, phi, ix, iy, iz, gx, gy, gz, lap);
+  T ph = phi[idx];
+  T s = ph * (T(1) - ph) * rsqrt_t(gx * gx + gy * gy + gz * gz + T(1e-24));
+  Q[idx] = s * gx;
+  Q[P.N + idx] = s * gy;
+  Q[2 * P.N + idx] = s * gz;
+}
+
+// ---- stage K4b: phi^{n+1} = phi - div(phi u) + D lap(phi) - kappa_AC div(Qs)   (Eq. 20, R16)
+template <typename T>
+__global__ void __launch_bounds__(256) k_allen_cahn_naive(DevParams<T> P, long long nodes,
+                                                          const T* __restrict__ S,
+                                                          const T* __restrict__ Q,
+                                                          T* __restrict__ phin) {
+  long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= nodes) return;
+  int ix, iy, iz;
+  node_coords(P, idx, ix, iy, iz);
+  const T* phi = S + F_PHI * P.N;
+  const T* u = S + F_UX * P.N;
+  T div = 0, sw = 0;
+#pragma unroll
+  for (int i = 0; i < 27; ++i) {
+    const int cx = i % 3 - 1, cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
+    int kx, ky, kz;
+    long long j = nbr(P, ix, iy, iz, cx, cy, cz, kx, ky, kz);
+    T w = w1<T>(cx) * w1<T>(cy) * w1<T>(cz);
+    T pj = phi[j];
+    sw = fma(w, pj, sw);
+    if (cx || cy || cz) {
+      // velocity-like ghosts: every component flips once per wall crossed (R19)
+      T s0 = ((kx + ky + kz) & 1) ? T(-1) : T(1);
+      T fl = 0;
+      if (cx) fl += T(cx) * (s0 * pj * u[j] + (kx ? -P.kappa_ac : P.kappa_ac) * Q[j]);
+      if (cy) fl += T(cy) * (s0 * pj * u[P.N + j] + (ky ? -P.kappa_ac : P.kappa_ac) * Q[P.N + j]);
+      if (cz) fl += T(cz) * (s0 * pj * u[2 * P.N + j] + (kz ? -P.kappa_ac : P.kappa_ac) * Q[2 * P.N + j]);
+      div = fma(w, fl, div);
+    }
+  }
+  T p0 = phi[idx];
+  phin[idx] = p0 - T(3) * div + P.mob * T(6) * (sw - p0);
+}
+
+// ---- stage K3+K1+K2: pull-stream with per-source reconstruction, moments, forces, closing
+template <typename T>
+__device__ __forceinline__ Coef<T> load_coef(const T* __restrict__ S, long long N, long long j) {
+  return coefficients<T>(S[F_P * N + j], S[F_UX * N + j], S[F_UY * N + j], S[F_UZ * N + j],
+                         S[F_AXX * N + j], S[F_AYY * N + j], S[F_AZZ * N + j], S[F_AXY * N + j],
+                         S[F_AXZ * N + j], S[F_AYZ * N + j], S[F_AX * N + j], S[F_AY * N + j],
+                         S[F_AZ * N + j]);
+}
+
+template <typename T, int I>
+__device__ __forceinline__ void pull_dir(const DevParams<T>& P, const T* __restrict__ S, int ix,
+                                         int iy, int iz, long long idx, const Coef<T>& self,
+                                         Mom<T>& m) {
+  constexpr int CX = I % 3 - 1, CY = (I / 3) % 3 - 1, CZ = I / 9 - 1;
+  int kx, ky, kz;
+  long long j = nbr(P, ix, iy, iz, -CX, -CY, -CZ, kx, ky, kz);
+  T f;
+  if (kx | ky | kz) {
+    f = fpost_dir<T, -CX, -CY, -CZ>(self);        // halfway bounce-back (R19)
+  } else if (CX == 0 && CY == 0 && CZ == 0) {
+    f = fpost_dir<T, 0, 0, 0>(self);
+  } else {
+    Coef<T> c = load_coef(S, P.N, j);
+    f = fpost_dir<T, CX, CY, CZ>(c);
+  }
+  accumulate<T, CX, CY, CZ>(m, f);
+  (void)idx;
+}
+
+template <typename T, int I>
+struct PullAll {
+  static __device__ __forceinline__ void run(const DevParams<T>& P, const T* __restrict__ S, int ix,
+                                             int iy, int iz, long long idx, const Coef<T>& self,
+                                             Mom<T>& m) {
+    pull_dir<T, I>(P, S, ix, iy, iz, idx, self, m);
+    PullAll<T, I + 1>::run(P, S, ix, iy, iz, idx, self, m);
+  }
+};
+template <typename T>
+struct PullAll<T, 27> {
+  static __device__ __forceinline__ void run(const DevParams<T>&, const T* __restrict__, int, int,
+                                             int, long long, const Coef<T>&, Mom<T>&) {}
+};
+
+template <typename T>
+__device__ __forceinline__ void store_node(T* __restrict__ D, long long N, long long idx,
+                                           const NodeOut<T>& o) {
+  D[F_P * N + idx] = o.p;
+  D[F_UX * N + idx] = o.ux; D[F_UY * N + idx] = o.uy; D[F_UZ * N + idx] = o.uz;
+  D[F_AXX * N + idx] = o.axx; D[F_AYY * N + idx] = o.ayy; D[F_AZZ * N + idx] = o.azz;
+  D[F_AXY * N + idx] = o.axy; D[F_AXZ * N + idx] = o.axz; D[F_AYZ * N + idx] = o.ayz;
+  D[F_AX * N + idx] = o.ax; D[F_AY * N + idx] = o.ay; D[F_AZ * N + idx] = o.az;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128) k_stream_collide_naive(DevParams<T> P, long long nodes,
+                                                              const T* __restrict__ S,
+                                                              T* __restrict__ D) {
+  long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= nodes) return;
+  int ix, iy, iz;
+  node_coords(P, idx, ix, iy, iz);
+  Coef<T> self = load_coef(S, P.N, idx);
+  Mom<T> m = {};
+  PullAll<T, 0>::run(P, S, ix, iy, iz, idx, self, m);
+  const T* phin = D + F_PHI * P.N;              // phi^{n+1}, written by the Allen-Cahn stage
+  T gx, gy, gz, lap;
+  grad_lap(P, phin, ix, iy, iz, gx, gy, gz, lap);
+  NodeOut<T> o = close_node(P, m, phin[idx], gx, gy, gz, lap, S[F_UX * P.N + idx],
+                            S[F_UY * P.N + idx], S[F_UZ * P.N + idx]);
+  store_node(D, P.N, idx, o);
+}
+
+// ---- tslb_init: p* = 0, Ahat = 0 (R9), a = (F^s + F^b)/rho from phi (R19 ghosts)
+template <typename T>
+__global__ void __launch_bounds__(256) k_init(DevParams<T> P, long long nodes,
+                                              const T* __restrict__ phi0,
+                                              const T* __restrict__ u0, long long us,
+                                              T* __restrict__ D) {
+  long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= nodes) return;
+  int ix, iy, iz;
+  node_coords(P, idx, ix, iy, iz);
+  T gx, gy, gz, lap;
+  grad_lap(P, phi0, ix, iy, iz, gx, gy, gz, lap);
+  T ph = phi0[idx];
+  Mix<T> mx = mixture(P, ph);
+  T mu_phi = P.beta4 * ph * (ph - T(1)) * (ph - T(0.5)) - P.kappa_mu * lap;
+  T db = mx.rho - P.rho_l;
+  NodeOut<T> o = {};
+  o.ux = u0[idx]; o.uy = u0[us + idx]; o.uz = u0[2 * us + idx];
+  o.ax = fma(db, P.gx, mu_phi * gx) * mx.inv_rho;
+  o.ay = fma(db, P.gy, mu_phi * gy) * mx.inv_rho;
+  o.az = fma(db, P.gz, mu_phi * gz) * mx.inv_rho;
+  store_node(D, P.N, idx, o);
+  D[F_PHI * P.N + idx] = ph;
+}
+
+// ---- tslb_get: rho, p = p* rho cs^2, u, phi
+template <typename T>
+__global__ void __launch_bounds__(256) k_get(DevParams<T> P, long long nodes,
+                                             const T* __restrict__ S, T* __restrict__ rho,
+                                             T* __restrict__ p, T* __restrict__ u, long long us,
+                                             T* __restrict__ phi) {
+  long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= nodes) return;
+  T ph = S[F_PHI * P.N + idx];
+  T r = fma(clamp01(ph), P.drho, P.rho_g);
+  if (rho) rho[idx] = r;
+  if (p) p[idx] = S[F_P * P.N + idx] * r * T(1.0 / 3.0);
+  if (u) {
+    u[idx] = S[F_UX * P.N + idx];
+    u[us + idx] = S[F_UY * P.N + idx];
+    u[2 * us + idx] = S[F_UZ * P.N + idx];
+  }
+  if (phi) phi[idx] = ph;
+}
+
+}  // namespace tslb

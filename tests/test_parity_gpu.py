@@ -1,0 +1,148 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Tolerances are BASELINE.json's: max|gpu-ref|/max|ref| <= 1e-10 per
+field in fp64, <= 1e-4 on u and phi in fp32."""
+import numpy as np
+import pytest
+
+from paper_2501_00846_b200 import inputs as I
+from parity_util import compare, rel_err, run_gpu, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+PATHS = {"naive": 1, "tiled": 0}            # TSLB_FLAG_NAIVE or the production kernels
+TOL64, TOL32 = 1e-10, 1e-4
+
+
+def _small_case(name):
+    if name == "ragged_periodic":            # several tiles in x and y plus a ragged tail
+        shape = (19, 21, 37)
+        prm = I.base_params()
+        phi = I.sphere_profile(shape, (17.0, 9.5, 8.0), 6.0, 4.0, prm["bc"])
+        u = I.noise_u(shape, 1e-3, 21)
+        steps = [1, 2, 50]
+    elif name == "bubble_walls_z":           # configs[2] in miniature: gravity + bounce-back
+        cfg = I.rising_bubble(nx=20, ny=12, nz=26, radius=5.0, height=9.0)
+        cfg["u"] = I.noise_u(cfg["shape"], 1e-4, 22)
+        return cfg, [1, 60]
+    elif name == "walls_all":                # droplet touching a corner, walls on every axis
+        shape = (8, 9, 10)
+        prm = I.base_params(bc=(1, 1, 1), body_accel=(1e-5, -2e-5, 3e-5))
+        phi = I.sphere_profile(shape, (2.0, 2.5, 1.5), 3.0, 4.0, prm["bc"])
+        u = I.noise_u(shape, 1e-3, 23)
+        steps = [1, 40]
+    elif name == "walls_xy":                 # walls on the tile axes, periodic marching axis
+        shape = (12, 7, 35)
+        prm = I.base_params(bc=(1, 1, 0), body_accel=(0.0, 0.0, 2e-5))
+        phi = I.sphere_profile(shape, (30.0, 3.0, 6.0), 4.0, 4.0, prm["bc"])
+        u = I.noise_u(shape, 1e-3, 24)
+        steps = [1, 40]
+    elif name == "min_periodic":             # smallest legal periodic box
+        shape = (4, 4, 4)
+        prm = I.base_params()
+        phi = I.sphere_profile(shape, (1.5, 1.5, 1.5), 1.2, 4.0, prm["bc"])
+        u = I.noise_u(shape, 1e-3, 25)
+        steps = [1, 30]
+    elif name == "min_walls":                # smallest legal box with walls everywhere
+        shape = (2, 2, 2)
+        prm = I.base_params(bc=(1, 1, 1))
+        phi = I.sphere_profile(shape, (0.0, 0.0, 0.0), 0.8, 4.0, prm["bc"])
+        u = I.noise_u(shape, 1e-3, 26)
+        steps = [1, 30]
+    else:
+        raise KeyError(name)
+    return dict(name=name, shape=shape, params=prm, phi=phi, u=u), steps
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config0_static_droplet_fp64(ref, path):
+    """BASELINE.json configs[0]: 32^3, 200 steps, fp64, error reported against step count."""
+    cfg = I.static_droplet(32, 8.0, seed=1)
+    steps = [1, 10, 100, 200]
+    want = run_oracle(ref, cfg, steps)
+    got, _ = run_gpu(cfg, steps, "f64", PATHS[path])
+    for n, g, r in zip(steps, got, want):
+        errs, bad = compare(ref, cfg, g, r, TOL64, state_tol=1e-9)
+        print(f"[{path}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+        assert not bad, (n, bad)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config0_static_droplet_fp32(ref, path):
+    cfg = I.static_droplet(32, 8.0, seed=1)
+    steps = [1, 200]
+    want = run_oracle(ref, cfg, steps)
+    got, _ = run_gpu(cfg, steps, "f32", PATHS[path])
+    for n, g, r in zip(steps, got, want):
+        errs, bad = compare(ref, cfg, g, r, TOL32, fields=("u", "phi"))
+        print(f"[{path}] fp32 step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+        assert not bad, (n, bad)
+        assert rel_err(g["rho"], r["rho"]) < 1e-3
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("case", ["ragged_periodic", "bubble_walls_z", "walls_all", "walls_xy",
+                                  "min_periodic", "min_walls"])
+def test_small_cases_fp64(ref, path, case):
+    cfg, steps = _small_case(case)
+    want = run_oracle(ref, cfg, steps)
+    got, _ = run_gpu(cfg, steps, "f64", PATHS[path])
+    for n, g, r in zip(steps, got, want):
+        errs, bad = compare(ref, cfg, g, r, TOL64, state_tol=1e-9)
+        print(f"[{path}/{case}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+        assert not bad, (case, n, bad)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("case", ["ragged_periodic", "bubble_walls_z", "walls_all"])
+def test_small_cases_fp32(ref, path, case):
+    cfg, steps = _small_case(case)
+    want = run_oracle(ref, cfg, steps)
+    got, _ = run_gpu(cfg, steps, "f32", PATHS[path])
+    for n, g, r in zip(steps, got, want):
+        errs, bad = compare(ref, cfg, g, r, TOL32, fields=("u", "phi"))
+        print(f"[{path}/{case}] fp32 step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+        assert not bad, (case, n, bad)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_laplace_128_short_fp64(ref, path):
+    """configs[1] geometry (128^3, R = 16) for a few steps: many tiles, many z chunks."""
+    cfg = I.static_droplet(128, 16.0, seed=16)
+    steps = [1, 4]
+    want = run_oracle(ref, cfg, steps)
+    got, _ = run_gpu(cfg, steps, "f64", PATHS[path])
+    for n, g, r in zip(steps, got, want):
+        errs, bad = compare(ref, cfg, g, r, TOL64, state_tol=1e-9)
+        print(f"[{path}] 128^3 step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+        assert not bad, (n, bad)
+
+
+def test_host_api_matches_device_api(ref):
+    """tslb_init_host / tslb_get_host (the e2e calls of bench.py) give the same fields."""
+    cfg, steps = _small_case("bubble_walls_z")
+    dev, _ = run_gpu(cfg, steps, "f64", 0)
+    host, _ = run_gpu(cfg, steps, "f64", 0, host_api=True)
+    for d, h in zip(dev, host):
+        for k in ("rho", "p", "u", "phi"):
+            assert np.array_equal(d[k], h[k]), k
+
+
+def test_step_zero_and_reinit():
+    from paper_2501_00846_b200 import binding as B
+    cfg = I.static_droplet(16, 4.0, seed=2)
+    s = B.Solver(16, 16, 16, cfg["params"])
+    s.init(cfg["phi"], cfg["u"])
+    a = {k: v.clone() for k, v in s.get().items()}
+    n0 = s.launches
+    s.step(0)
+    assert s.launches == n0
+    s.step(7)
+    b = {k: v.clone() for k, v in s.get().items()}
+    s.init(cfg["phi"], cfg["u"])                 # restart
+    c = s.get()
+    s.step(7)
+    d = s.get()
+    s.synchronize()
+    for k in a:
+        assert bool((a[k] == c[k]).all()) and bool((b[k] == d[k]).all()), k
+    s.close()
