@@ -36,6 +36,8 @@ def parse():
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
                     help="precision of the headline value (the other one is reported beside it)")
     ap.add_argument("--naive", action="store_true", help="time the validation kernels instead")
+    ap.add_argument("--variant", type=int, default=0, help="tuning variant (flags bits 8-15)")
+    ap.add_argument("--generic", action="store_true", help="force the wall-capable tiled kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--only", default=None, choices=[None, "f64", "f32"],
@@ -243,7 +245,7 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
-    flags = 1 if args.naive else 0
+    flags = (1 if args.naive else 0) | (2 if args.generic else 0) | (args.variant << 8)
     cfg = make_workload(args.size)
     n = int(np.prod(cfg["shape"]))
     peak, peak_kind = peaks()
@@ -290,7 +292,8 @@ def main():
                 "scaling": "weak", "vs_baseline": None, "dtype": order[0], "data": "synthetic",
                 "config": {"workload": cfg["name"], "grid": list(cfg["shape"][::-1]),
                            "parallelism": f"replicas x{world}", "l2": "state 3.8 GB (f64) >> L2",
-                           "path": "naive" if args.naive else "tiled"},
+                           "path": "naive" if args.naive else ("tiled-generic" if args.generic else "tiled"),
+                           "variant": args.variant},
                 "clocks": head["clocks"], "gpu_launches": head["launches"],
                 "roofline": head["roofline"], "finite": head["finite"],
                 "phi_drift": head["phi_drift"]}

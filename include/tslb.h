@@ -40,8 +40,12 @@ enum { TSLB_OK = 0, TSLB_EINVAL = -1, TSLB_EWORKSPACE = -2, TSLB_ECUDA = -3, TSL
 
 /* flags (bit field) */
 enum {
-  TSLB_FLAG_NAIVE = 1 /* run the one-thread-per-node global-memory kernels (debug/validation
-                         path, same arithmetic contract); default 0 = tiled z-marching kernels */
+  TSLB_FLAG_NAIVE = 1,   /* run the one-thread-per-node global-memory kernels (debug/validation
+                            path, same arithmetic contract); default 0 = tiled z-marching kernels */
+  TSLB_FLAG_GENERIC = 2, /* on an all-periodic box, run the wall-capable tiled kernel instead of
+                            the lean periodic one (validation of the former at full size)        */
+  TSLB_FLAG_VARIANT_MASK = 0xff00 /* bits 8-15: tuning variant of the lean kernel (tile height,
+                            blocks per SM, prefetch); 0 = the production choice                  */
 };
 
 typedef struct tslb_params {

@@ -12,7 +12,7 @@
 
 #include "tslb_device.cuh"
 #include "tslb_naive.cuh"
-#include "tslb_tiled.cuh"
+#include "tslb_launch.cuh"
 
 namespace {
 
@@ -38,7 +38,7 @@ bool params_ok(int nx, int ny, int nz, const tslb_params* p) {
         p->mobility > 0 && p->sigma >= 0))
     return false;
   if (p->precision != TSLB_F32 && p->precision != TSLB_F64) return false;
-  if (p->flags & ~TSLB_FLAG_NAIVE) return false;
+  if (p->flags & ~(TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC | TSLB_FLAG_VARIANT_MASK)) return false;
   const int n[3] = {nx, ny, nz};
   for (int d = 0; d < 3; ++d) {
     if (p->bc[d] != TSLB_BC_PERIODIC && p->bc[d] != TSLB_BC_WALL) return false;
@@ -162,7 +162,8 @@ int step_impl(tslb_handle* h, int n, const tslb::Marker& mk) {
       mk.mark(TSLB_K_STREAM_COLLIDE);
       h->launches += 3;
     } else {
-      int rc = tslb::launch_step_tiled<T>(P, S, D, h->stream, &h->launches, mk);
+      int rc = tslb::launch_step_tiled<T>(P, S, D, h->stream, &h->launches, mk,
+                                           h->prm.flags);
       if (rc != 0) return fail(TSLB_ECUDA, "tiled launch: %s", cudaGetErrorString(cudaError_t(rc)));
     }
     h->cur ^= 1;
@@ -235,17 +236,20 @@ int tslb_get(tslb_handle* h, void* rho, void* p, void* u, void* phi) {
 int tslb_get_state(tslb_handle* h, void* pstar, void* u, void* A, void* a, void* phi) {
   if (!h) return fail(TSLB_EINVAL, "tslb_get_state: NULL handle");
   if (!h->inited) return fail(TSLB_ESTATE, "tslb_get_state before tslb_init");
-  const char* S = h->buf[h->cur];
-  const size_t pb = size_t(h->stride) * h->es, nb = size_t(h->nodes) * h->es;
-  struct { void* dst; int first, count; } parts[5] = {
-      {pstar, tslb::F_P, 1}, {u, tslb::F_UX, 3}, {A, tslb::F_AXX, 6}, {a, tslb::F_AX, 3},
-      {phi, tslb::F_PHI, 1}};
-  for (auto& q : parts) {
-    if (!q.dst) continue;
-    for (int k = 0; k < q.count; ++k)
-      CUDA_TRY(cudaMemcpyAsync(static_cast<char*>(q.dst) + nb * k, S + pb * (q.first + k), nb,
-                               cudaMemcpyDeviceToDevice, h->stream));
+  unsigned blocks = unsigned((h->nodes + 255) / 256);
+  if (h->prm.precision == TSLB_F64) {
+    auto P = make_dev<double>(h->nx, h->ny, h->nz, h->prm, h->stride);
+    tslb::k_get_state<double><<<blocks, 256, 0, h->stream>>>(
+        P, h->nodes, reinterpret_cast<const double*>(h->buf[h->cur]), (double*)pstar, (double*)u,
+        (double*)A, (double*)a, (double*)phi);
+  } else {
+    auto P = make_dev<float>(h->nx, h->ny, h->nz, h->prm, h->stride);
+    tslb::k_get_state<float><<<blocks, 256, 0, h->stream>>>(
+        P, h->nodes, reinterpret_cast<const float*>(h->buf[h->cur]), (float*)pstar, (float*)u,
+        (float*)A, (float*)a, (float*)phi);
   }
+  h->launches += 1;
+  CUDA_TRY(cudaGetLastError());
   return TSLB_OK;
 }
 

@@ -24,10 +24,68 @@ struct Marker {
   }
 };
 
-// Stored state per node: 14 SoA planes in this order.
+// Stored state per node: 14 scalars, indexed in this order everywhere in the code:
 //   0 p*   1-3 u   4-9 Ahat = (1 - omega(phi)) a2_neq (xx,yy,zz,xy,xz,yz)   10-12 a = F/rho   13 phi
 enum { F_P = 0, F_UX = 1, F_UY = 2, F_UZ = 3, F_AXX = 4, F_AYY = 5, F_AZZ = 6, F_AXY = 7,
        F_AXZ = 8, F_AYZ = 9, F_AX = 10, F_AY = 11, F_AZ = 12, F_PHI = 13, NFIELD = 14 };
+
+// HBM layout: one buffer = 14 N scalars (N = padded node count).
+// Fields 0..11 are interleaved per node in 128-bit vectors so that a thread moves them with
+// 128-bit loads/stores and a warp touches 512 contiguous bytes per instruction:
+//   fp64: 6 planes of double2  (p*,ux) (uy,uz) (Axx,Ayy) (Azz,Axy) (Axz,Ayz) (ax,ay)
+//   fp32: 3 planes of float4   (p*,ux,uy,uz) (Axx,Ayy,Azz,Axy) (Axz,Ayz,ax,ay)
+// followed by the scalar plane az (offset 12 N) and the scalar plane phi (offset 13 N), which
+// the Allen-Cahn kernel writes on its own.
+template <typename T> struct VecOf;
+template <> struct VecOf<double> { using type = double2; static constexpr int W = 2; };
+template <> struct VecOf<float> { using type = float4; static constexpr int W = 4; };
+
+__device__ __forceinline__ void unpack(const double2& v, double* m) { m[0] = v.x; m[1] = v.y; }
+__device__ __forceinline__ void unpack(const float4& v, float* m) {
+  m[0] = v.x; m[1] = v.y; m[2] = v.z; m[3] = v.w;
+}
+__device__ __forceinline__ double2 pack(const double* m) { return make_double2(m[0], m[1]); }
+__device__ __forceinline__ float4 pack(const float* m) { return make_float4(m[0], m[1], m[2], m[3]); }
+
+// the 13 moment scalars (fields 0..12) of node idx
+template <typename T>
+__device__ __forceinline__ void load13(const T* __restrict__ S, long long N, long long idx,
+                                       T (&m)[13]) {
+  using V = typename VecOf<T>::type;
+  constexpr int W = VecOf<T>::W;
+  const V* g = reinterpret_cast<const V*>(S);
+#pragma unroll
+  for (int k = 0; k < 12 / W; ++k) unpack(__ldg(g + k * N + idx), &m[k * W]);
+  m[12] = __ldg(S + 12 * N + idx);
+}
+template <typename T>
+__device__ __forceinline__ void store13(T* __restrict__ D, long long N, long long idx,
+                                        const T (&m)[13]) {
+  using V = typename VecOf<T>::type;
+  constexpr int W = VecOf<T>::W;
+  V* g = reinterpret_cast<V*>(D);
+#pragma unroll
+  for (int k = 0; k < 12 / W; ++k) g[k * N + idx] = pack(&m[k * W]);
+  D[12 * N + idx] = m[12];
+}
+// velocity only (Allen-Cahn stage): 2 x 128 bit in fp64, 1 x 128 bit in fp32
+__device__ __forceinline__ void load_u(const double* __restrict__ S, long long N, long long idx,
+                                       double& ux, double& uy, double& uz) {
+  const double2* g = reinterpret_cast<const double2*>(S);
+  const double2 a = __ldg(g + idx), b = __ldg(g + N + idx);
+  ux = a.y; uy = b.x; uz = b.y;
+}
+__device__ __forceinline__ void load_u(const float* __restrict__ S, long long N, long long idx,
+                                       float& ux, float& uy, float& uz) {
+  const float4 a = __ldg(reinterpret_cast<const float4*>(S) + idx);
+  ux = a.y; uy = a.z; uz = a.w;
+}
+// element offset of one scalar field of node idx (slow path: init / get / naive kernels)
+template <typename T>
+__device__ __forceinline__ long long field_off(long long N, long long idx, int f) {
+  constexpr int W = VecOf<T>::W;
+  return f < 12 ? (long long)(f / W) * W * N + idx * W + (f % W) : (long long)f * N + idx;
+}
 
 template <typename T>
 struct DevParams {
@@ -184,6 +242,18 @@ __device__ __forceinline__ NodeOut<T> close_node(const DevParams<T>& P, const Mo
   o.axz = om1 * (m.xz - o.ux * o.uz + h * (o.ux * o.az + o.ax * o.uz));
   o.ayz = om1 * (m.yz - o.uy * o.uz + h * (o.uy * o.az + o.ay * o.uz));
   return o;
+}
+
+template <typename T>
+__device__ __forceinline__ void store_out(T* __restrict__ D, long long N, long long idx,
+                                          const NodeOut<T>& o) {
+  const T m[13] = {o.p, o.ux, o.uy, o.uz, o.axx, o.ayy, o.azz, o.axy, o.axz, o.ayz, o.ax, o.ay, o.az};
+  store13(D, N, idx, m);
+}
+template <typename T>
+__device__ __forceinline__ Coef<T> coef_from13(const T (&m)[13]) {
+  return coefficients<T>(m[F_P], m[F_UX], m[F_UY], m[F_UZ], m[F_AXX], m[F_AYY], m[F_AZZ], m[F_AXY],
+                         m[F_AXZ], m[F_AYZ], m[F_AX], m[F_AY], m[F_AZ]);
 }
 
 // Ghost rule along one axis (R19): periodic wrap or even mirror about a wall half a cell outside

@@ -1,0 +1,274 @@
+// tslb_fast.cuh -- lean stream-collide kernel for all-periodic boxes.
+//
+// Same tiling as tslb_tiled.cuh, but the arithmetic uses the tensor-product structure of D3Q27:
+//   * the post-collision population of a node is the polynomial  w(c) P(c),
+//       P(cx,cy,cz) = E(cx,cy) + cz O(cx,cy) + (cz^2 - 1/3) Qq(cx,cy)          (Eq. 7-10, 14)
+//     so the source evaluates the three in-plane fields E, O, Qq (9 values each) instead of 27
+//     populations, and ships E, O, Qq of the 8 moving in-plane directions through shared memory;
+//   * the lattice weights are products of (1,4,1)/6 per axis, so the receiver applies them while
+//     it reduces (adds become FMAs with the constant 4) and the common factor 1/216 is folded
+//     into the source's constants;
+//   * raw moments (Eq. 11-13) are linear in the populations, so the receiver reduces the FIELDS
+//     (3 x 17 operations) and only then forms the cz = +1 / 0 / -1 combinations.
+#pragma once
+#include "tslb_device.cuh"
+#include "tslb_tiled.cuh"
+
+namespace tslb {
+
+__host__ __device__ constexpr int dir_slot(int cx, int cy) {
+  int q = (cy + 1) * 3 + (cx + 1);
+  return q > 4 ? q - 1 : q;
+}
+
+// Exchange buffers, double buffered over the marching index so that one __syncthreads per plane
+// is enough.  fp64: (E,O) as one 128-bit word + Qq as a 64-bit word per direction and cell;
+// fp32: (E,O,Qq,-) as one 128-bit word.
+template <typename T, int CELLS> struct ExBuf;
+template <int CELLS> struct ExBuf<double, CELLS> {
+  double2 eo[8][CELLS];
+  double q[8][CELLS];
+  double2 pd[CELLS];      // (pz, dz) of phi^{n+1}: (phi(z-1)+phi(z+1)) + 4 phi(z),  phi(z+1) - phi(z-1)
+  __device__ __forceinline__ void put(int slot, int c, double E, double O, double Q) {
+    eo[slot][c] = make_double2(E, O);
+    q[slot][c] = Q;
+  }
+  __device__ __forceinline__ void get(int slot, int c, double& E, double& O, double& Q) const {
+    const double2 v = eo[slot][c];
+    E = v.x; O = v.y; Q = q[slot][c];
+  }
+  __device__ __forceinline__ void put_pd(int c, double a, double b) { pd[c] = make_double2(a, b); }
+  __device__ __forceinline__ void get_pd(int c, double& a, double& b) const {
+    const double2 v = pd[c]; a = v.x; b = v.y;
+  }
+};
+template <int CELLS> struct ExBuf<float, CELLS> {
+  float4 eoq[8][CELLS];
+  float2 pd[CELLS];
+  __device__ __forceinline__ void put(int slot, int c, float E, float O, float Q) {
+    eoq[slot][c] = make_float4(E, O, Q, 0.f);
+  }
+  __device__ __forceinline__ void get(int slot, int c, float& E, float& O, float& Q) const {
+    const float4 v = eoq[slot][c];
+    E = v.x; O = v.y; Q = v.z;
+  }
+  __device__ __forceinline__ void put_pd(int c, float a, float b) { pd[c] = make_float2(a, b); }
+  __device__ __forceinline__ void get_pd(int c, float& a, float& b) const {
+    const float2 v = pd[c]; a = v.x; b = v.y;
+  }
+};
+template <typename T, int CELLS>
+struct K2FastSmem { ExBuf<T, CELLS> buf[2]; };
+
+// E, O, Qq on the 3x3 in-plane directions, index [cx+1][cy+1], all scaled by 1/216.
+template <typename T> struct SrcFields { T E[3][3], O[3][3], Q[3][3]; };
+
+template <typename T>
+__device__ __forceinline__ void source_fields(const Coef<T>& c, SrcFields<T>& s) {
+  const T k = T(1.0 / 216.0);
+  T a0[3], a1[3], a2[3];
+  {   // E = a0(cx) + cy a1(cx) + (cy^2 - 1/3) a2(cx)
+    const T m0 = k * c.c0;
+    a0[1] = fma(T(-1.5) * k, c.xx, m0);
+    const T t = fma(T(3) * k, c.xx, m0);
+    a0[0] = fma(T(-3) * k, c.c1x, t);
+    a0[2] = fma(T(3) * k, c.c1x, t);
+    const T m1 = (T(3) * k) * c.c1y;
+    a1[1] = fma(T(-4.5) * k, c.xxy, m1);
+    const T t1 = fma(T(9) * k, c.xxy, m1);
+    a1[0] = fma(T(-9) * k, c.xy, t1);
+    a1[2] = fma(T(9) * k, c.xy, t1);
+    a2[1] = (T(4.5) * k) * c.yy;
+    a2[0] = fma(T(-13.5) * k, c.xyy, a2[1]);
+    a2[2] = fma(T(13.5) * k, c.xyy, a2[1]);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      s.E[i][1] = fma(T(-1.0 / 3.0), a2[i], a0[i]);
+      const T te = fma(T(2.0 / 3.0), a2[i], a0[i]);
+      s.E[i][0] = te - a1[i];
+      s.E[i][2] = te + a1[i];
+    }
+  }
+  {   // O = b0(cx) + cy b1(cx) + (cy^2 - 1/3) b2
+    const T m0 = (T(3) * k) * c.c1z;
+    a0[1] = fma(T(-4.5) * k, c.xxz, m0);
+    const T t = fma(T(9) * k, c.xxz, m0);
+    a0[0] = fma(T(-9) * k, c.xz, t);
+    a0[2] = fma(T(9) * k, c.xz, t);
+    a1[1] = (T(9) * k) * c.yz;
+    a1[0] = fma(T(-27) * k, c.xyz, a1[1]);
+    a1[2] = fma(T(27) * k, c.xyz, a1[1]);
+    const T b2 = (T(13.5) * k) * c.yyz;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      s.O[i][1] = fma(T(-1.0 / 3.0), b2, a0[i]);
+      const T to = fma(T(2.0 / 3.0), b2, a0[i]);
+      s.O[i][0] = to - a1[i];
+      s.O[i][2] = to + a1[i];
+    }
+  }
+  {   // Qq = d0(cx) + cy d1
+    a0[1] = (T(4.5) * k) * c.zz;
+    a0[0] = fma(T(-13.5) * k, c.xzz, a0[1]);
+    a0[2] = fma(T(13.5) * k, c.xzz, a0[1]);
+    const T d1 = (T(13.5) * k) * c.yzz;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      s.Q[i][1] = a0[i];
+      s.Q[i][0] = a0[i] - d1;
+      s.Q[i][2] = a0[i] + d1;
+    }
+  }
+}
+
+// In-plane moments {1, x, y, xx, yy, xy} of a field given on the 3x3 arrival directions, with the
+// lattice weights (1,4,1) (x) (1,4,1) (the factor 1/36 lives in the source constants).
+template <typename T> struct Red6 { T s1, sx, sy, sxx, syy, sxy; };
+
+template <typename T>
+__device__ __forceinline__ Red6<T> reduce6(const T (&v)[3][3]) {   // v[cx+1][cy+1]
+  T r0[3], r1[3], r2[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    r2[i] = v[i][2] + v[i][0];
+    r1[i] = v[i][2] - v[i][0];
+    r0[i] = fma(T(4), v[i][1], r2[i]);
+  }
+  Red6<T> r;
+  r.sxx = r0[2] + r0[0];
+  r.sx = r0[2] - r0[0];
+  r.s1 = fma(T(4), r0[1], r.sxx);
+  r.sxy = r1[2] - r1[0];
+  r.sy = fma(T(4), r1[1], r1[2] + r1[0]);
+  r.syy = fma(T(4), r2[1], r2[2] + r2[0]);
+  return r;
+}
+
+template <typename T, int TX, int TY, int MINB, bool PREFETCH>
+__global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
+k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D, int zchunk) {
+  using M = TileMap<TX, TY, 1>;
+  using SM = K2FastSmem<T, M::CELLS>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SM& sm = *reinterpret_cast<SM*>(smem_raw);
+
+  const int tid = threadIdx.x;
+  int lx, ly;
+  const bool mapped = M::coords(tid, lx, ly);
+  const int gx = blockIdx.x * TX + lx, gy = blockIdx.y * TY + ly;
+  const int z0 = blockIdx.z * zchunk;
+  const int z1 = min(P.nz, z0 + zchunk);
+  const int c = M::cell(lx, ly);
+  const bool in_ring = mapped && gx >= -1 && gx <= P.nx && gy >= -1 && gy <= P.ny;
+  const bool is_out = tid < M::NMAIN && gx < P.nx && gy < P.ny;
+  const int sx = gx < 0 ? gx + P.nx : (gx >= P.nx ? gx - P.nx : gx);      // periodic wrap
+  const int sy = gy < 0 ? gy + P.ny : (gy >= P.ny ? gy - P.ny : gy);
+  const int plane = P.nx * P.ny;
+  const int col = in_ring ? sx + P.nx * sy : 0;
+  const T* phin = D + F_PHI * P.N;
+
+  // register pipeline along z (destination planes j-1 = "A", j = "B")
+  T accA[6] = {}, accB[6] = {}, zoA[3] = {}, zoB[3] = {};
+  T ph_m = 0, ph_0 = 0, ph_p = 0;
+  T uo[2][3] = {};
+  T nxt[13], nxt_phi = 0;                      // prefetched state of the next source plane
+
+  auto load_plane = [&](int j, T (&m)[13], T& ph) {
+    const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
+    const long long s = col + (long long)plane * jz;
+    load13(S, P.N, s, m);
+    ph = __ldg(phin + s);
+  };
+  if (PREFETCH && in_ring) load_plane(z0 - 1, nxt, nxt_phi);
+
+  for (int j = z0 - 1; j <= z1; ++j) {
+    ExBuf<T, M::CELLS>& xb = sm.buf[(j - z0 + 1) & 1];
+    T ownE = 0, ownO = 0, ownQ = 0;
+    ph_m = ph_0; ph_0 = ph_p;
+    uo[0][0] = uo[1][0]; uo[0][1] = uo[1][1]; uo[0][2] = uo[1][2];
+    if (in_ring) {
+      T cur[13];
+      if (PREFETCH) {
+#pragma unroll
+        for (int f = 0; f < 13; ++f) cur[f] = nxt[f];
+        ph_p = nxt_phi;
+      } else {
+        load_plane(j, cur, ph_p);
+      }
+      uo[1][0] = cur[F_UX]; uo[1][1] = cur[F_UY]; uo[1][2] = cur[F_UZ];
+      const Coef<T> cf = coef_from13(cur);
+      SrcFields<T> sf;
+      source_fields(cf, sf);
+      ownE = sf.E[1][1]; ownO = sf.O[1][1]; ownQ = sf.Q[1][1];
+#pragma unroll
+      for (int q = 0; q < 9; ++q) {
+        const int cx = q % 3 - 1, cy = q / 3 - 1;
+        if (cx == 0 && cy == 0) continue;
+        xb.put(dir_slot(cx, cy), c, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
+      }
+      xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
+    }
+    __syncthreads();
+    if (PREFETCH && in_ring && j < z1) load_plane(j + 1, nxt, nxt_phi);
+
+    if (is_out) {
+      T vE[3][3], vO[3][3], vQ[3][3];
+      vE[1][1] = ownE; vO[1][1] = ownO; vQ[1][1] = ownQ;
+#pragma unroll
+      for (int q = 0; q < 9; ++q) {
+        const int cx = q % 3 - 1, cy = q / 3 - 1;
+        if (cx == 0 && cy == 0) continue;
+        xb.get(dir_slot(cx, cy), c - cy * M::W - cx, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1],
+               vQ[cx + 1][cy + 1]);
+      }
+      const Red6<T> rE = reduce6(vE), rO = reduce6(vO), rQ = reduce6(vQ);
+      const T e[6] = {rE.s1, rE.sx, rE.sy, rE.sxx, rE.syy, rE.sxy};
+      const T o[6] = {rO.s1, rO.sx, rO.sy, rO.sxx, rO.syy, rO.sxy};
+      const T qq[6] = {rQ.s1, rQ.sx, rQ.sy, rQ.sxx, rQ.syy, rQ.sxy};
+      T up[6], dn[6];
+#pragma unroll
+      for (int i = 0; i < 6; ++i) {
+        const T t = fma(T(2.0 / 3.0), qq[i], e[i]);          // cz = +-1 : E + (2/3) Qq +- O
+        up[i] = t + o[i];
+        dn[i] = t - o[i];
+        accA[i] += dn[i];                                    // arrives at plane j-1
+        accB[i] += fma(T(-4.0 / 3.0), qq[i], T(4) * e[i]);   // cz = 0 : 4 (E - Qq/3)
+      }
+      const int k = j - 1;
+      if (k >= z0) {
+        Mom<T> m;
+        m.p = accA[0]; m.mx = accA[1]; m.my = accA[2];
+        m.xx = accA[3]; m.yy = accA[4]; m.xy = accA[5];
+        m.mz = zoA[0] - dn[0]; m.xz = zoA[1] - dn[1]; m.yz = zoA[2] - dn[2];
+        m.zz = zoA[0] + dn[0];
+        // separable gradient / Laplacian of phi^{n+1} at plane k (Eq. 18, repaired Eq. 19)
+        T rs[3], rd[3], zs[3];
+#pragma unroll
+        for (int r = 0; r < 3; ++r) {
+          const int cc = c + (r - 1) * M::W;
+          T am, a0, ap, bm, b0, bp;
+          xb.get_pd(cc - 1, am, bm);
+          xb.get_pd(cc, a0, b0);
+          xb.get_pd(cc + 1, ap, bp);
+          rs[r] = fma(T(4), a0, am + ap);
+          rd[r] = ap - am;
+          zs[r] = fma(T(4), b0, bm + bp);
+        }
+        const T sw = fma(T(4), rs[1], rs[0] + rs[2]);
+        const T gx_ = fma(T(4), rd[1], rd[0] + rd[2]) * T(3.0 / 216.0);
+        const T gy_ = (rs[2] - rs[0]) * T(3.0 / 216.0);
+        const T gz_ = fma(T(4), zs[1], zs[0] + zs[2]) * T(3.0 / 216.0);
+        const T lap = fma(T(6.0 / 216.0), sw, T(-6) * ph_0);
+        const NodeOut<T> out =
+            close_node(P, m, ph_0, gx_, gy_, gz_, lap, uo[0][0], uo[0][1], uo[0][2]);
+        store_out(D, P.N, gx + P.nx * gy + (long long)plane * k, out);
+      }
+#pragma unroll
+      for (int i = 0; i < 6; ++i) { accA[i] = accB[i]; accB[i] = up[i]; }
+#pragma unroll
+      for (int i = 0; i < 3; ++i) { zoA[i] = zoB[i]; zoB[i] = up[i]; }
+    }
+  }
+}
+
+}  // namespace tslb

@@ -1,0 +1,91 @@
+// tslb_launch.cuh -- launch of one time step: kernel selection, grid sizing, attributes.
+#pragma once
+#include "tslb_fast.cuh"
+#include "tslb_tiled.cuh"
+
+namespace tslb {
+
+constexpr int ZCHUNK = 32;   // planes marched by one block (2 extra source planes per chunk)
+
+template <typename K>
+inline cudaError_t prepare(K kernel, size_t smem) {
+  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       int(smem));
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout,
+                              cudaSharedmemCarveoutMaxShared);
+}
+
+template <typename T, int TY, int MINB, bool PREFETCH>
+cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream) {
+  constexpr int TX = 32;
+  using M = TileMap<TX, TY, 1>;
+  auto kernel = k_stream_collide_fast<T, TX, TY, MINB, PREFETCH>;
+  const size_t smem = sizeof(K2FastSmem<T, M::CELLS>);
+  static bool ready = false;
+  if (!ready) {
+    cudaError_t e = prepare(kernel, smem);
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
+  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, ZCHUNK);
+  return cudaGetLastError();
+}
+
+template <typename T, bool WALLS>
+cudaError_t launch_generic(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream) {
+  constexpr int TX = 32, TY = 8;
+  using M = TileMap<TX, TY, 1>;
+  auto kernel = k_stream_collide_tiled<T, TX, TY, WALLS, 1>;
+  const size_t smem = sizeof(K2Smem<T, TX, TY>);
+  static bool ready = false;
+  if (!ready) {
+    cudaError_t e = prepare(kernel, smem);
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
+  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, ZCHUNK);
+  return cudaGetLastError();
+}
+
+// variant = (flags >> 8) & 0xff : tuning selector, 0 = production choice.
+template <typename T>
+int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream,
+                      long long* launches, const Marker& mk, int flags) {
+  const bool walls = P.bcx || P.bcy || P.bcz;
+  const bool generic = walls || (flags & 2);
+  const int variant = (flags >> 8) & 0xff;
+  {
+    constexpr int TX = 32, TY = 8;
+    using M1 = TileMap<TX, TY, 2>;
+    const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
+    k_allen_cahn_tiled<T, TX, TY, 2><<<grid, M1::NTHREADS, 0, stream>>>(P, S, D + F_PHI * P.N,
+                                                                        ZCHUNK);
+    mk.mark(1);
+  }
+  cudaError_t e;
+  if (generic) {
+    e = walls ? launch_generic<T, true>(P, S, D, stream) : launch_generic<T, false>(P, S, D, stream);
+  } else {
+    switch (variant) {
+      default:   // production choice: fp64 one block/SM, fp32 two blocks/SM
+      case 0:
+        e = sizeof(T) == 8 ? launch_fast<T, 8, 1, true>(P, S, D, stream)
+                           : launch_fast<T, 8, 2, true>(P, S, D, stream);
+        break;
+      case 6: e = launch_fast<T, 8, 1, false>(P, S, D, stream); break;
+      case 1: e = launch_fast<T, 8, 1, true>(P, S, D, stream); break;
+      case 2: e = launch_fast<T, 8, 2, false>(P, S, D, stream); break;
+      case 3: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, false>(P, S, D, stream); break;
+      case 4: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, true>(P, S, D, stream); break;
+      case 5: e = launch_fast<T, 8, 2, true>(P, S, D, stream); break;
+    }
+  }
+  mk.mark(2);
+  *launches += 2;
+  return int(e);
+}
+
+}  // namespace tslb

@@ -78,7 +78,6 @@ __global__ void __launch_bounds__(256) k_allen_cahn_naive(DevParams<T> P, long l
   int ix, iy, iz;
   node_coords(P, idx, ix, iy, iz);
   const T* phi = S + F_PHI * P.N;
-  const T* u = S + F_UX * P.N;
   T div = 0, sw = 0;
 #pragma unroll
   for (int i = 0; i < 27; ++i) {
@@ -91,10 +90,11 @@ __global__ void __launch_bounds__(256) k_allen_cahn_naive(DevParams<T> P, long l
     if (cx || cy || cz) {
       // velocity-like ghosts: every component flips once per wall crossed (R19)
       T s0 = ((kx + ky + kz) & 1) ? T(-1) : T(1);
-      T fl = 0;
-      if (cx) fl += T(cx) * (s0 * pj * u[j] + (kx ? -P.kappa_ac : P.kappa_ac) * Q[j]);
-      if (cy) fl += T(cy) * (s0 * pj * u[P.N + j] + (ky ? -P.kappa_ac : P.kappa_ac) * Q[P.N + j]);
-      if (cz) fl += T(cz) * (s0 * pj * u[2 * P.N + j] + (kz ? -P.kappa_ac : P.kappa_ac) * Q[2 * P.N + j]);
+      T fl = 0, ux, uy, uz;
+      load_u(S, P.N, j, ux, uy, uz);
+      if (cx) fl += T(cx) * (s0 * pj * ux + (kx ? -P.kappa_ac : P.kappa_ac) * Q[j]);
+      if (cy) fl += T(cy) * (s0 * pj * uy + (ky ? -P.kappa_ac : P.kappa_ac) * Q[P.N + j]);
+      if (cz) fl += T(cz) * (s0 * pj * uz + (kz ? -P.kappa_ac : P.kappa_ac) * Q[2 * P.N + j]);
       div = fma(w, fl, div);
     }
   }
@@ -105,10 +105,9 @@ __global__ void __launch_bounds__(256) k_allen_cahn_naive(DevParams<T> P, long l
 // ---- stage K3+K1+K2: pull-stream with per-source reconstruction, moments, forces, closing
 template <typename T>
 __device__ __forceinline__ Coef<T> load_coef(const T* __restrict__ S, long long N, long long j) {
-  return coefficients<T>(S[F_P * N + j], S[F_UX * N + j], S[F_UY * N + j], S[F_UZ * N + j],
-                         S[F_AXX * N + j], S[F_AYY * N + j], S[F_AZZ * N + j], S[F_AXY * N + j],
-                         S[F_AXZ * N + j], S[F_AYZ * N + j], S[F_AX * N + j], S[F_AY * N + j],
-                         S[F_AZ * N + j]);
+  T m[13];
+  load13(S, N, j, m);
+  return coef_from13(m);
 }
 
 template <typename T, int I>
@@ -149,11 +148,7 @@ struct PullAll<T, 27> {
 template <typename T>
 __device__ __forceinline__ void store_node(T* __restrict__ D, long long N, long long idx,
                                            const NodeOut<T>& o) {
-  D[F_P * N + idx] = o.p;
-  D[F_UX * N + idx] = o.ux; D[F_UY * N + idx] = o.uy; D[F_UZ * N + idx] = o.uz;
-  D[F_AXX * N + idx] = o.axx; D[F_AYY * N + idx] = o.ayy; D[F_AZZ * N + idx] = o.azz;
-  D[F_AXY * N + idx] = o.axy; D[F_AXZ * N + idx] = o.axz; D[F_AYZ * N + idx] = o.ayz;
-  D[F_AX * N + idx] = o.ax; D[F_AY * N + idx] = o.ay; D[F_AZ * N + idx] = o.az;
+  store_out(D, N, idx, o);
 }
 
 template <typename T>
@@ -170,8 +165,9 @@ __global__ void __launch_bounds__(128) k_stream_collide_naive(DevParams<T> P, lo
   const T* phin = D + F_PHI * P.N;              // phi^{n+1}, written by the Allen-Cahn stage
   T gx, gy, gz, lap;
   grad_lap(P, phin, ix, iy, iz, gx, gy, gz, lap);
-  NodeOut<T> o = close_node(P, m, phin[idx], gx, gy, gz, lap, S[F_UX * P.N + idx],
-                            S[F_UY * P.N + idx], S[F_UZ * P.N + idx]);
+  T uox, uoy, uoz;
+  load_u(S, P.N, idx, uox, uoy, uoz);
+  NodeOut<T> o = close_node(P, m, phin[idx], gx, gy, gz, lap, uox, uoy, uoz);
   store_node(D, P.N, idx, o);
 }
 
@@ -211,13 +207,32 @@ __global__ void __launch_bounds__(256) k_get(DevParams<T> P, long long nodes,
   T ph = S[F_PHI * P.N + idx];
   T r = fma(clamp01(ph), P.drho, P.rho_g);
   if (rho) rho[idx] = r;
-  if (p) p[idx] = S[F_P * P.N + idx] * r * T(1.0 / 3.0);
+  if (p) p[idx] = S[field_off<T>(P.N, idx, F_P)] * r * T(1.0 / 3.0);
   if (u) {
-    u[idx] = S[F_UX * P.N + idx];
-    u[us + idx] = S[F_UY * P.N + idx];
-    u[2 * us + idx] = S[F_UZ * P.N + idx];
+    T ux, uy, uz;
+    load_u(S, P.N, idx, ux, uy, uz);
+    u[idx] = ux; u[us + idx] = uy; u[2 * us + idx] = uz;
   }
   if (phi) phi[idx] = ph;
 }
 
+}  // namespace tslb
+
+namespace tslb {
+// ---- tslb_get_state: de-interleave the stored fields into plain planes (NULL = skip)
+template <typename T>
+__global__ void __launch_bounds__(256) k_get_state(DevParams<T> P, long long nodes,
+                                                   const T* __restrict__ S, T* __restrict__ pstar,
+                                                   T* __restrict__ u, T* __restrict__ A,
+                                                   T* __restrict__ a, T* __restrict__ phi) {
+  long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= nodes) return;
+  T m[13];
+  load13(S, P.N, idx, m);
+  if (pstar) pstar[idx] = m[F_P];
+  if (u) for (int k = 0; k < 3; ++k) u[k * nodes + idx] = m[F_UX + k];
+  if (A) for (int k = 0; k < 6; ++k) A[k * nodes + idx] = m[F_AXX + k];
+  if (a) for (int k = 0; k < 3; ++k) a[k * nodes + idx] = m[F_AX + k];
+  if (phi) phi[idx] = S[F_PHI * P.N + idx];
+}
 }  // namespace tslb

@@ -184,12 +184,10 @@ k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ 
     uo[0][0] = uo[1][0]; uo[0][1] = uo[1][1]; uo[0][2] = uo[1][2];
     if (has_mom && plane_real) {
       const long long s = col + plane * jz;
-      const T ux = S[F_UX * P.N + s], uy = S[F_UY * P.N + s], uz = S[F_UZ * P.N + s];
-      Coef<T> cf = coefficients<T>(S[F_P * P.N + s], ux, uy, uz, S[F_AXX * P.N + s],
-                                   S[F_AYY * P.N + s], S[F_AZZ * P.N + s], S[F_AXY * P.N + s],
-                                   S[F_AXZ * P.N + s], S[F_AYZ * P.N + s], S[F_AX * P.N + s],
-                                   S[F_AY * P.N + s], S[F_AZ * P.N + s]);
-      uo[1][0] = ux; uo[1][1] = uy; uo[1][2] = uz;
+      T m13[13];
+      load13(S, P.N, s, m13);
+      Coef<T> cf = coef_from13(m13);
+      uo[1][0] = m13[F_UX]; uo[1][1] = m13[F_UY]; uo[1][2] = m13[F_UZ];
       K2StoreAll<T, TX, TY>::run(sm, c, cf, own);
     }
     // z-combinations of phi^{n+1} for the output plane k = j-1 (Eq. 18-19 are separable)
@@ -219,11 +217,7 @@ k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ 
         NodeOut<T> o = close_node(P, mom[0], ph_0, T(3) * sx_, T(3) * sy_, T(3) * sz_, lap,
                                   uo[0][0], uo[0][1], uo[0][2]);
         const long long d = gx + (long long)P.nx * gy + plane * k;
-        D[F_P * P.N + d] = o.p;
-        D[F_UX * P.N + d] = o.ux; D[F_UY * P.N + d] = o.uy; D[F_UZ * P.N + d] = o.uz;
-        D[F_AXX * P.N + d] = o.axx; D[F_AYY * P.N + d] = o.ayy; D[F_AZZ * P.N + d] = o.azz;
-        D[F_AXY * P.N + d] = o.axy; D[F_AXZ * P.N + d] = o.axz; D[F_AYZ * P.N + d] = o.ayz;
-        D[F_AX * P.N + d] = o.ax; D[F_AY * P.N + d] = o.ay; D[F_AZ * P.N + d] = o.az;
+        store_out(D, P.N, d, o);
       }
       mom[0] = mom[1]; mom[1] = mom[2]; mom[2] = Mom<T>{};
     }
@@ -238,18 +232,49 @@ k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ 
 // Ghost columns/planes beyond a wall are evaluated from mirrored inputs (phi even, u odd), which
 // yields the odd normal component of the sharpening flux that R19 prescribes.
 // ------------------------------------------------------------------------------------------
-template <typename T, int TX, int TY>
-struct K1Smem {
-  using M = TileMap<TX, TY, 2>;
-  T pz[M::CELLS], dz[M::CELLS];            // z-combinations of phi^n at the flux plane j
-  T X[M::CELLS], Y[M::CELLS], Z[M::CELLS]; // z-combinations of Q at the output plane k
+// Shared-memory cells of K1, double buffered along the marching index (one barrier per plane).
+template <typename T, int CELLS> struct K1Buf;
+template <int CELLS> struct K1Buf<double, CELLS> {
+  double2 pd[CELLS];                 // z-combinations of phi^n at a flux plane (x6, see below)
+  double2 xy[CELLS];                 // z-combinations of Qx, Qy at an output plane (x6)
+  double zz[CELLS];                  // z-combination of Qz at an output plane (x6)
+  __device__ __forceinline__ void put_pd(int c, double a, double b) { pd[c] = make_double2(a, b); }
+  __device__ __forceinline__ void get_pd(int c, double& a, double& b) const {
+    const double2 v = pd[c]; a = v.x; b = v.y;
+  }
+  __device__ __forceinline__ void put_q(int c, double x, double y, double z) {
+    xy[c] = make_double2(x, y); zz[c] = z;
+  }
+  __device__ __forceinline__ void get_q(int c, double& x, double& y, double& z) const {
+    const double2 v = xy[c]; x = v.x; y = v.y; z = zz[c];
+  }
+};
+template <int CELLS> struct K1Buf<float, CELLS> {
+  float2 pd[CELLS];
+  float4 q[CELLS];
+  __device__ __forceinline__ void put_pd(int c, float a, float b) { pd[c] = make_float2(a, b); }
+  __device__ __forceinline__ void get_pd(int c, float& a, float& b) const {
+    const float2 v = pd[c]; a = v.x; b = v.y;
+  }
+  __device__ __forceinline__ void put_q(int c, float x, float y, float z) {
+    q[c] = make_float4(x, y, z, 0.f);
+  }
+  __device__ __forceinline__ void get_q(int c, float& x, float& y, float& z) const {
+    const float4 v = q[c]; x = v.x; y = v.y; z = v.z;
+  }
 };
 
+// Software pipeline of iteration j (all inside one barrier interval):
+//   (a) ring-2 threads publish the z-combinations of phi^n for plane j+1,
+//   (b) ring-1 threads turn the combinations of plane j (published one iteration ago) into the
+//       flux Q(j) and publish the z-combinations of Q for plane j-1,
+//   (c) main threads turn the combinations of Q for plane j-2 into phi^{n+1}(j-2).
+// Global loads (phi two planes ahead, u one plane ahead) are issued one iteration before use.
 template <typename T, int TX, int TY, int MINB>
 __global__ void __launch_bounds__((TileMap<TX, TY, 2>::NTHREADS), MINB)
 k_allen_cahn_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ phin, int zchunk) {
   using M = TileMap<TX, TY, 2>;
-  __shared__ K1Smem<T, TX, TY> sm;
+  __shared__ K1Buf<T, M::CELLS> sm[2];
 
   const int tid = threadIdx.x;
   int lx, ly;
@@ -266,118 +291,97 @@ k_allen_cahn_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ phin
   int kx = 0, ky = 0;
   const int sx = ghost_index(min(max(gx, -2), P.nx + 1), P.nx, P.bcx, kx);
   const int sy = ghost_index(min(max(gy, -2), P.ny + 1), P.ny, P.bcy, ky);
-  const long long col = sx + (long long)P.nx * sy;
-  const long long plane = (long long)P.nx * P.ny;
+  const int col = sx + P.nx * sy;
+  const int plane = P.nx * P.ny;
   const T* phi = S + F_PHI * P.N;
-  const T* u = S + F_UX * P.N;
 
-  int kz;
-  T q_m = 0, q_0 = 0, q_p = 0;                 // phi^n at planes j-1, j, j+1 of the own column
+  auto load_phi = [&](int z) {
+    int kz;
+    return __ldg(phi + col + (long long)plane * ghost_index(z, P.nz, P.bcz, kz));
+  };
+  // phi u at plane z with velocity-like ghosts (sign flips once per wall crossed, R19)
+  auto load_u = [&](int z, T& ux, T& uy, T& uz) {
+    int kz;
+    const int jz = ghost_index(z, P.nz, P.bcz, kz);
+    tslb::load_u(S, P.N, col + (long long)plane * jz, ux, uy, uz);
+    if ((kx + ky + kz) & 1) { ux = -ux; uy = -uy; uz = -uz; }
+  };
+
+  // phi^n of the own column at planes j, j+1, j+2 (after the shift inside iteration j)
+  T f0 = 0, f1 = 0, f2 = 0, fn = 0;
+  T un[3] = {};                                  // prefetched u of the next flux plane
+  T Qa[3] = {}, Qb[3] = {};                      // Q at planes j-2, j-1
+  T sw1 = 0, sw2 = 0, ph1 = 0, ph2 = 0;          // smoothing of pz and phi at planes j-1, j-2
+
+  // prologue: publish plane z0-1, prefetch what iteration z0-1 consumes
   if (ring2) {
-    q_0 = phi[col + plane * ghost_index(z0 - 2, P.nz, P.bcz, kz)];
-    q_p = phi[col + plane * ghost_index(z0 - 1, P.nz, P.bcz, kz)];
+    const T a = load_phi(z0 - 2);
+    f1 = load_phi(z0 - 1);
+    f2 = load_phi(z0);
+    fn = load_phi(z0 + 1);
+    sm[0].put_pd(c, fma(T(4), f1, a + f2), f2 - a);
   }
-  T Qa[3] = {}, Qb[3] = {}, Qc[3] = {};        // Q at planes j-2, j-1, j
-  T sw_prev = 0, phi_prev = 0;                 // in-plane smoothing of pz and phi at plane j-1
+  if (ring1) load_u(z0 - 1, un[0], un[1], un[2]);
+  __syncthreads();
 
-  for (int j = z0 - 1; j <= z1; ++j) {
-    q_m = q_0; q_0 = q_p;
-    if (ring2) {
-      q_p = phi[col + plane * ghost_index(j + 1, P.nz, P.bcz, kz)];
-      sm.pz[c] = T(1.0 / 6.0) * (q_m + q_p) + T(2.0 / 3.0) * q_0;
-      sm.dz[c] = T(1.0 / 6.0) * (q_p - q_m);
+  for (int j = z0 - 1; j <= z1 + 1; ++j) {
+    const int b = (j - z0 + 1) & 1;
+    // (a) publish plane j+1
+    f0 = f1; f1 = f2; f2 = fn;
+    if (ring2 && j + 1 <= z1) {
+      sm[b ^ 1].put_pd(c, fma(T(4), f1, f0 + f2), f2 - f0);
+      if (j + 3 <= z1 + 1) fn = load_phi(j + 3);
     }
-    __syncthreads();
-
-    T sw_now = 0;
-    if (ring1) {
-      T sx_ = 0, sy_ = 0, sz_ = 0;
+    // (b) flux of plane j, z-combinations of Q for plane j-1
+    T sw0 = 0;
+    if (ring1 && j <= z1) {
+      const T u0 = un[0], u1 = un[1], u2 = un[2];
+      if (j + 1 <= z1) load_u(j + 1, un[0], un[1], un[2]);
+      T rs[3], rd[3], zs[3];
 #pragma unroll
-      for (int q = 0; q < 9; ++q) {
-        const int cx = q % 3 - 1, cy = q / 3 - 1;
-        const T w = w1<T>(cx) * w1<T>(cy);
-        const T a = sm.pz[c + cy * M::W + cx], b = sm.dz[c + cy * M::W + cx];
-        sw_now = fma(w, a, sw_now);
-        sz_ = fma(w, b, sz_);
-        if (cx) sx_ = fma(w * T(cx), a, sx_);
-        if (cy) sy_ = fma(w * T(cy), a, sy_);
+      for (int r = 0; r < 3; ++r) {
+        const int cc = c + (r - 1) * M::W;
+        T am, a0, ap, bm, b0, bp;
+        sm[b].get_pd(cc - 1, am, bm);
+        sm[b].get_pd(cc, a0, b0);
+        sm[b].get_pd(cc + 1, ap, bp);
+        rs[r] = fma(T(4), a0, am + ap);
+        rd[r] = ap - am;
+        zs[r] = fma(T(4), b0, bm + bp);
       }
-      const T g0 = T(3) * sx_, g1 = T(3) * sy_, g2 = T(3) * sz_;
-      const T s = P.kappa_ac * q_0 * (T(1) - q_0) *
-                  rsqrt_t(g0 * g0 + g1 * g1 + g2 * g2 + T(1e-24));
-      const int jz = ghost_index(j, P.nz, P.bcz, kz);
-      const long long n = col + plane * jz;
-      const T sgn = ((kx + ky + kz) & 1) ? -q_0 : q_0;      // phi u with velocity-like ghosts
-#pragma unroll
-      for (int al = 0; al < 3; ++al) { Qa[al] = Qb[al]; Qb[al] = Qc[al]; }
-      Qc[0] = fma(sgn, u[n], s * g0);
-      Qc[1] = fma(sgn, u[P.N + n], s * g1);
-      Qc[2] = fma(sgn, u[2 * P.N + n], s * g2);
-      // z-combinations of Q for the output plane k = j-1 (Eq. 18, component-wise: R17)
-      sm.X[c] = T(1.0 / 6.0) * (Qa[0] + Qc[0]) + T(2.0 / 3.0) * Qb[0];
-      sm.Y[c] = T(1.0 / 6.0) * (Qa[1] + Qc[1]) + T(2.0 / 3.0) * Qb[1];
-      sm.Z[c] = T(1.0 / 6.0) * (Qc[2] - Qa[2]);
+      sw0 = fma(T(4), rs[1], rs[0] + rs[2]);
+      const T g0 = fma(T(4), rd[1], rd[0] + rd[2]) * T(3.0 / 216.0);
+      const T g1 = (rs[2] - rs[0]) * T(3.0 / 216.0);
+      const T g2 = fma(T(4), zs[1], zs[0] + zs[2]) * T(3.0 / 216.0);
+      const T s = P.kappa_ac * f0 * (T(1) - f0) * rsqrt_t(g0 * g0 + g1 * g1 + g2 * g2 + T(1e-24));
+      const T Qc0 = fma(f0, u0, s * g0), Qc1 = fma(f0, u1, s * g1), Qc2 = fma(f0, u2, s * g2);
+      sm[b].put_q(c, fma(T(4), Qb[0], Qa[0] + Qc0), fma(T(4), Qb[1], Qa[1] + Qc1), Qc2 - Qa[2]);
+      Qa[0] = Qb[0]; Qa[1] = Qb[1]; Qa[2] = Qb[2];
+      Qb[0] = Qc0; Qb[1] = Qc1; Qb[2] = Qc2;
     }
-    __syncthreads();
-
-    const int k = j - 1;
+    // (c) output plane k = j-2 from the combinations published one iteration ago
+    const int k = j - 2;
     if (is_out && k >= z0) {
-      T div = 0;
+      T rx[3], ry[3], rz[3];
 #pragma unroll
-      for (int q = 0; q < 9; ++q) {
-        const int cx = q % 3 - 1, cy = q / 3 - 1;
-        const T w = w1<T>(cx) * w1<T>(cy);
-        const int cc = c + cy * M::W + cx;
-        div = fma(w, sm.Z[cc], div);
-        if (cx) div = fma(w * T(cx), sm.X[cc], div);
-        if (cy) div = fma(w * T(cy), sm.Y[cc], div);
+      for (int r = 0; r < 3; ++r) {
+        const int cc = c + (r - 1) * M::W;
+        T xm, ym, zm, x0, y0, z0_, xp, yp, zp;
+        sm[b ^ 1].get_q(cc - 1, xm, ym, zm);
+        sm[b ^ 1].get_q(cc, x0, y0, z0_);
+        sm[b ^ 1].get_q(cc + 1, xp, yp, zp);
+        rx[r] = xp - xm;
+        ry[r] = fma(T(4), y0, ym + yp);
+        rz[r] = fma(T(4), z0_, zm + zp);
       }
-      const T lap = T(6) * (sw_prev - phi_prev);
-      phin[gx + (long long)P.nx * gy + plane * k] = phi_prev - T(3) * div + P.mob * lap;
+      // div Q = 3/216 [ (1,4,1)_y (x) d_x X + d_y (x) (1,4,1)_x Y + (1,4,1)^2 Z ]
+      const T div = fma(T(4), rx[1], rx[0] + rx[2]) + (ry[2] - ry[0]) + fma(T(4), rz[1], rz[0] + rz[2]);
+      const T lap = fma(T(6.0 / 216.0), sw2, T(-6) * ph2);
+      phin[gx + P.nx * gy + (long long)plane * k] = ph2 - T(3.0 / 216.0) * div + P.mob * lap;
     }
-    sw_prev = sw_now;
-    phi_prev = q_0;
+    sw2 = sw1; sw1 = sw0; ph2 = ph1; ph1 = f0;
+    __syncthreads();
   }
-}
-
-// ------------------------------------------------------------------------------------------
-// Launch of one time step.
-// ------------------------------------------------------------------------------------------
-template <typename T> struct TileCfg;
-template <> struct TileCfg<double> { static constexpr int TX = 32, TY = 8, ZC = 32; };
-template <> struct TileCfg<float>  { static constexpr int TX = 32, TY = 8, ZC = 32; };
-
-template <typename T>
-int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream,
-                      long long* launches, const Marker& mk) {
-  constexpr int TX = TileCfg<T>::TX, TY = TileCfg<T>::TY, ZC = TileCfg<T>::ZC;
-  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZC - 1) / ZC);
-  using M1 = TileMap<TX, TY, 2>;
-  using M2 = TileMap<TX, TY, 1>;
-  const bool walls = P.bcx || P.bcy || P.bcz;
-
-  k_allen_cahn_tiled<T, TX, TY, 1><<<grid, M1::NTHREADS, 0, stream>>>(P, S, D + F_PHI * P.N, ZC);
-  mk.mark(1);
-
-  const size_t smem2 = sizeof(K2Smem<T, TX, TY>);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e;
-    e = cudaFuncSetAttribute(k_stream_collide_tiled<T, TX, TY, false, 1>,
-                             cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem2));
-    if (e != cudaSuccess) return int(e);
-    e = cudaFuncSetAttribute(k_stream_collide_tiled<T, TX, TY, true, 1>,
-                             cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem2));
-    if (e != cudaSuccess) return int(e);
-    attr_set = true;
-  }
-  if (walls)
-    k_stream_collide_tiled<T, TX, TY, true, 1><<<grid, M2::NTHREADS, smem2, stream>>>(P, S, D, ZC);
-  else
-    k_stream_collide_tiled<T, TX, TY, false, 1><<<grid, M2::NTHREADS, smem2, stream>>>(P, S, D, ZC);
-  mk.mark(2);
-  *launches += 2;
-  return int(cudaGetLastError());
 }
 
 }  // namespace tslb

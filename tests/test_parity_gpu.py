@@ -121,6 +121,25 @@ def test_laplace_128_short_fp64(ref, path):
         assert not bad, (n, bad)
 
 
+@pytest.mark.parametrize("flags", [2] + [v << 8 for v in range(7)])
+def test_kernel_variants_fp64(ref, flags):
+    """Every tuning variant of the lean periodic kernel (flags bits 8-15) and the wall-capable
+    kernel forced onto a periodic box (TSLB_FLAG_GENERIC) meet the same bar."""
+    cfg, steps = _small_case("ragged_periodic")
+    cfg["shape"] = (40, 37, 70)                     # 3 x 5 tiles of 32 x 8, two z chunks, ragged
+    cfg["phi"] = I.sphere_profile(cfg["shape"], (30.3, 16.1, 19.7), 9.0, 4.0)
+    cfg["u"] = I.noise_u(cfg["shape"], 1e-3, 31)
+    steps = [1, 12]
+    want = run_oracle(ref, cfg, steps)
+    for prec, tol, fields in (("f64", TOL64, ("rho", "p", "u", "phi")), ("f32", TOL32, ("u", "phi"))):
+        got, _ = run_gpu(cfg, steps, prec, flags)
+        for n, g, r in zip(steps, got, want):
+            errs, bad = compare(ref, cfg, g, r, tol, fields=fields,
+                                state_tol=1e-9 if prec == "f64" else None)
+            print(f"[flags={flags:#x} {prec}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+            assert not bad, (flags, prec, n, bad)
+
+
 def test_host_api_matches_device_api(ref):
     """tslb_init_host / tslb_get_host (the e2e calls of bench.py) give the same fields."""
     cfg, steps = _small_case("bubble_walls_z")
