@@ -37,6 +37,7 @@ def parse():
                     help="precision of the headline value (the other one is reported beside it)")
     ap.add_argument("--naive", action="store_true", help="time the validation kernels instead")
     ap.add_argument("--variant", type=int, default=0, help="tuning variant (flags bits 8-15)")
+    ap.add_argument("--k1variant", type=int, default=0, help="Allen-Cahn tuning variant (bits 16-19)")
     ap.add_argument("--generic", action="store_true", help="force the wall-capable tiled kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -245,7 +246,7 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
-    flags = (1 if args.naive else 0) | (2 if args.generic else 0) | (args.variant << 8)
+    flags = (1 if args.naive else 0) | (2 if args.generic else 0) | (args.variant << 8) | (args.k1variant << 16)
     cfg = make_workload(args.size)
     n = int(np.prod(cfg["shape"]))
     peak, peak_kind = peaks()

@@ -37,6 +37,10 @@ template <int CELLS> struct ExBuf<double, CELLS> {
     const double2 v = eo[slot][c];
     E = v.x; O = v.y; Q = q[slot][c];
   }
+  __device__ __forceinline__ void get_eo(int slot, int c, double& E, double& O) const {
+    const double2 v = eo[slot][c]; E = v.x; O = v.y;
+  }
+  __device__ __forceinline__ void get_q(int slot, int c, double& Q) const { Q = q[slot][c]; }
   __device__ __forceinline__ void put_pd(int c, double a, double b) { pd[c] = make_double2(a, b); }
   __device__ __forceinline__ void get_pd(int c, double& a, double& b) const {
     const double2 v = pd[c]; a = v.x; b = v.y;
@@ -52,6 +56,10 @@ template <int CELLS> struct ExBuf<float, CELLS> {
     const float4 v = eoq[slot][c];
     E = v.x; O = v.y; Q = v.z;
   }
+  __device__ __forceinline__ void get_eo(int slot, int c, float& E, float& O) const {
+    const float4 v = eoq[slot][c]; E = v.x; O = v.y;
+  }
+  __device__ __forceinline__ void get_q(int slot, int c, float& Q) const { Q = eoq[slot][c].z; }
   __device__ __forceinline__ void put_pd(int c, float a, float b) { pd[c] = make_float2(a, b); }
   __device__ __forceinline__ void get_pd(int c, float& a, float& b) const {
     const float2 v = pd[c]; a = v.x; b = v.y;
@@ -167,25 +175,25 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   const int col = in_ring ? sx + P.nx * sy : 0;
   const T* phin = D + F_PHI * P.N;
 
-  // register pipeline along z (destination planes j-1 = "A", j = "B")
-  T accA[6] = {}, accB[6] = {}, zoA[3] = {}, zoB[3] = {};
+  // Register pipeline along z.  Two slots alternate roles every plane ("A" = destination plane
+  // j-1, completed in iteration j; "B" = destination plane j), so the marching loop is unrolled
+  // by two and no register is moved to shift the pipeline.
+  T acc0[6] = {}, acc1[6] = {}, zo0[3] = {}, zo1[3] = {}, u0[3] = {}, u1[3] = {};
   T ph_m = 0, ph_0 = 0, ph_p = 0;
-  T uo[2][3] = {};
   T nxt[13], nxt_phi = 0;                      // prefetched state of the next source plane
 
   auto load_plane = [&](int j, T (&m)[13], T& ph) {
     const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
-    const long long s = col + (long long)plane * jz;
+    const int s = col + plane * jz;
     load13(S, P.N, s, m);
     ph = __ldg(phin + s);
   };
   if (PREFETCH && in_ring) load_plane(z0 - 1, nxt, nxt_phi);
 
-  for (int j = z0 - 1; j <= z1; ++j) {
-    ExBuf<T, M::CELLS>& xb = sm.buf[(j - z0 + 1) & 1];
+  auto body = [&](const int j, ExBuf<T, M::CELLS>& xb, T (&aA)[6], T (&aB)[6], T (&zA)[3],
+                  T (&zB)[3], const T (&uPrev)[3], T (&uCur)[3]) {
     T ownE = 0, ownO = 0, ownQ = 0;
     ph_m = ph_0; ph_0 = ph_p;
-    uo[0][0] = uo[1][0]; uo[0][1] = uo[1][1]; uo[0][2] = uo[1][2];
     if (in_ring) {
       T cur[13];
       if (PREFETCH) {
@@ -195,7 +203,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
       } else {
         load_plane(j, cur, ph_p);
       }
-      uo[1][0] = cur[F_UX]; uo[1][1] = cur[F_UY]; uo[1][2] = cur[F_UZ];
+      uCur[0] = cur[F_UX]; uCur[1] = cur[F_UY]; uCur[2] = cur[F_UZ];
       const Coef<T> cf = coef_from13(cur);
       SrcFields<T> sf;
       source_fields(cf, sf);
@@ -212,35 +220,52 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
     if (PREFETCH && in_ring && j < z1) load_plane(j + 1, nxt, nxt_phi);
 
     if (is_out) {
-      T vE[3][3], vO[3][3], vQ[3][3];
-      vE[1][1] = ownE; vO[1][1] = ownO; vQ[1][1] = ownQ;
+      Red6<T> rE, rO, rQ;
+      {
+        T vE[3][3], vO[3][3];
+        vE[1][1] = ownE; vO[1][1] = ownO;
 #pragma unroll
-      for (int q = 0; q < 9; ++q) {
-        const int cx = q % 3 - 1, cy = q / 3 - 1;
-        if (cx == 0 && cy == 0) continue;
-        xb.get(dir_slot(cx, cy), c - cy * M::W - cx, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1],
-               vQ[cx + 1][cy + 1]);
+        for (int q = 0; q < 9; ++q) {
+          const int cx = q % 3 - 1, cy = q / 3 - 1;
+          if (cx == 0 && cy == 0) continue;
+          xb.get_eo(dir_slot(cx, cy), c - cy * M::W - cx, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
+        }
+        rE = reduce6(vE);
+        rO = reduce6(vO);
       }
-      const Red6<T> rE = reduce6(vE), rO = reduce6(vO), rQ = reduce6(vQ);
+      if (sizeof(T) == 8) asm volatile("" ::: "memory");   // keep the Qq loads behind the E/O work
+      {
+        T vQ[3][3];
+        vQ[1][1] = ownQ;
+#pragma unroll
+        for (int q = 0; q < 9; ++q) {
+          const int cx = q % 3 - 1, cy = q / 3 - 1;
+          if (cx == 0 && cy == 0) continue;
+          xb.get_q(dir_slot(cx, cy), c - cy * M::W - cx, vQ[cx + 1][cy + 1]);
+        }
+        rQ = reduce6(vQ);
+      }
       const T e[6] = {rE.s1, rE.sx, rE.sy, rE.sxx, rE.syy, rE.sxy};
       const T o[6] = {rO.s1, rO.sx, rO.sy, rO.sxx, rO.syy, rO.sxy};
       const T qq[6] = {rQ.s1, rQ.sx, rQ.sy, rQ.sxx, rQ.syy, rQ.sxy};
-      T up[6], dn[6];
+      T up[6], dn[3];
 #pragma unroll
       for (int i = 0; i < 6; ++i) {
         const T t = fma(T(2.0 / 3.0), qq[i], e[i]);          // cz = +-1 : E + (2/3) Qq +- O
         up[i] = t + o[i];
-        dn[i] = t - o[i];
-        accA[i] += dn[i];                                    // arrives at plane j-1
-        accB[i] += fma(T(-4.0 / 3.0), qq[i], T(4) * e[i]);   // cz = 0 : 4 (E - Qq/3)
+        const T d = t - o[i];
+        if (i < 3) dn[i] = d;
+        aA[i] += d;                                          // arrives at plane j-1
+        aB[i] += fma(T(-4.0 / 3.0), qq[i], T(4) * e[i]);     // cz = 0 : 4 (E - Qq/3)
       }
       const int k = j - 1;
       if (k >= z0) {
         Mom<T> m;
-        m.p = accA[0]; m.mx = accA[1]; m.my = accA[2];
-        m.xx = accA[3]; m.yy = accA[4]; m.xy = accA[5];
-        m.mz = zoA[0] - dn[0]; m.xz = zoA[1] - dn[1]; m.yz = zoA[2] - dn[2];
-        m.zz = zoA[0] + dn[0];
+        m.p = aA[0]; m.mx = aA[1]; m.my = aA[2];
+        m.xx = aA[3]; m.yy = aA[4]; m.xy = aA[5];
+        m.mz = zA[0] - dn[0]; m.xz = zA[1] - dn[1]; m.yz = zA[2] - dn[2];
+        m.zz = zA[0] + dn[0];
+        if (sizeof(T) == 8) asm volatile("" ::: "memory");
         // separable gradient / Laplacian of phi^{n+1} at plane k (Eq. 18, repaired Eq. 19)
         T rs[3], rd[3], zs[3];
 #pragma unroll
@@ -259,15 +284,20 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         const T gy_ = (rs[2] - rs[0]) * T(3.0 / 216.0);
         const T gz_ = fma(T(4), zs[1], zs[0] + zs[2]) * T(3.0 / 216.0);
         const T lap = fma(T(6.0 / 216.0), sw, T(-6) * ph_0);
-        const NodeOut<T> out =
-            close_node(P, m, ph_0, gx_, gy_, gz_, lap, uo[0][0], uo[0][1], uo[0][2]);
-        store_out(D, P.N, gx + P.nx * gy + (long long)plane * k, out);
+        const NodeOut<T> out = close_node(P, m, ph_0, gx_, gy_, gz_, lap, uPrev[0], uPrev[1], uPrev[2]);
+        store_out(D, P.N, gx + P.nx * gy + plane * k, out);
       }
+      // slot A is free now: it becomes the accumulator of destination plane j+1
 #pragma unroll
-      for (int i = 0; i < 6; ++i) { accA[i] = accB[i]; accB[i] = up[i]; }
+      for (int i = 0; i < 6; ++i) aA[i] = up[i];
 #pragma unroll
-      for (int i = 0; i < 3; ++i) { zoA[i] = zoB[i]; zoB[i] = up[i]; }
+      for (int i = 0; i < 3; ++i) zA[i] = up[i];
     }
+  };
+
+  for (int j = z0 - 1; j <= z1; j += 2) {
+    body(j, sm.buf[0], acc0, acc1, zo0, zo1, u0, u1);
+    if (j + 1 <= z1) body(j + 1, sm.buf[1], acc1, acc0, zo1, zo0, u1, u0);
   }
 }
 

@@ -50,6 +50,29 @@ cudaError_t launch_generic(const DevParams<T>& P, const T* S, T* D, cudaStream_t
   return cudaGetLastError();
 }
 
+template <typename T, int TY, int MINB, bool WALLS>
+cudaError_t launch_k1w(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream) {
+  constexpr int TX = 32;
+  using M = TileMap<TX, TY, 2>;
+  auto kernel = k_allen_cahn_tiled<T, TX, TY, MINB, WALLS>;
+  const size_t smem = 2 * sizeof(K1Buf<T, M::CELLS>);
+  static bool ready = false;
+  if (!ready) {
+    cudaError_t e = prepare(kernel, smem);
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
+  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D + F_PHI * P.N, ZCHUNK);
+  return cudaGetLastError();
+}
+
+template <typename T, int TY, int MINB>
+cudaError_t launch_k1(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream) {
+  return (P.bcx || P.bcy || P.bcz) ? launch_k1w<T, TY, MINB, true>(P, S, D, stream)
+                                   : launch_k1w<T, TY, MINB, false>(P, S, D, stream);
+}
+
 // variant = (flags >> 8) & 0xff : tuning selector, 0 = production choice.
 template <typename T>
 int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream,
@@ -57,15 +80,16 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, cudaStream_t stre
   const bool walls = P.bcx || P.bcy || P.bcz;
   const bool generic = walls || (flags & 2);
   const int variant = (flags >> 8) & 0xff;
-  {
-    constexpr int TX = 32, TY = 8;
-    using M1 = TileMap<TX, TY, 2>;
-    const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
-    k_allen_cahn_tiled<T, TX, TY, 2><<<grid, M1::NTHREADS, 0, stream>>>(P, S, D + F_PHI * P.N,
-                                                                        ZCHUNK);
-    mk.mark(1);
-  }
   cudaError_t e;
+  switch ((flags >> 16) & 0xf) {     // bits 16-19: tuning variant of the Allen-Cahn kernel
+    default:
+    case 0: e = launch_k1<T, 8, 2>(P, S, D, stream); break;
+    case 1: e = launch_k1<T, 16, 1>(P, S, D, stream); break;
+    case 2: e = launch_k1<T, 8, 1>(P, S, D, stream); break;
+    case 3: e = launch_k1<T, 4, 3>(P, S, D, stream); break;
+  }
+  if (e != cudaSuccess) return int(e);
+  mk.mark(1);
   if (generic) {
     e = walls ? launch_generic<T, true>(P, S, D, stream) : launch_generic<T, false>(P, S, D, stream);
   } else {
@@ -73,9 +97,12 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, cudaStream_t stre
       default:   // production choice: fp64 one block/SM, fp32 two blocks/SM
       case 0:
         e = sizeof(T) == 8 ? launch_fast<T, 8, 1, true>(P, S, D, stream)
-                           : launch_fast<T, 8, 2, true>(P, S, D, stream);
+                           : launch_fast<T, 8, 2, false>(P, S, D, stream);
         break;
       case 6: e = launch_fast<T, 8, 1, false>(P, S, D, stream); break;
+      case 7: e = launch_fast<T, 4, 2, false>(P, S, D, stream); break;
+      case 8: e = launch_fast<T, 4, 2, true>(P, S, D, stream); break;
+      case 9: e = launch_fast<T, 4, 3, false>(P, S, D, stream); break;
       case 1: e = launch_fast<T, 8, 1, true>(P, S, D, stream); break;
       case 2: e = launch_fast<T, 8, 2, false>(P, S, D, stream); break;
       case 3: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, false>(P, S, D, stream); break;

@@ -233,48 +233,31 @@ k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ 
 // yields the odd normal component of the sharpening flux that R19 prescribes.
 // ------------------------------------------------------------------------------------------
 // Shared-memory cells of K1, double buffered along the marching index (one barrier per plane).
-template <typename T, int CELLS> struct K1Buf;
-template <int CELLS> struct K1Buf<double, CELLS> {
-  double2 pd[CELLS];                 // z-combinations of phi^n at a flux plane (x6, see below)
-  double2 xy[CELLS];                 // z-combinations of Qx, Qy at an output plane (x6)
-  double zz[CELLS];                  // z-combination of Qz at an output plane (x6)
-  __device__ __forceinline__ void put_pd(int c, double a, double b) { pd[c] = make_double2(a, b); }
-  __device__ __forceinline__ void get_pd(int c, double& a, double& b) const {
-    const double2 v = pd[c]; a = v.x; b = v.y;
-  }
-  __device__ __forceinline__ void put_q(int c, double x, double y, double z) {
-    xy[c] = make_double2(x, y); zz[c] = z;
-  }
-  __device__ __forceinline__ void get_q(int c, double& x, double& y, double& z) const {
-    const double2 v = xy[c]; x = v.x; y = v.y; z = zz[c];
-  }
-};
-template <int CELLS> struct K1Buf<float, CELLS> {
-  float2 pd[CELLS];
-  float4 q[CELLS];
-  __device__ __forceinline__ void put_pd(int c, float a, float b) { pd[c] = make_float2(a, b); }
-  __device__ __forceinline__ void get_pd(int c, float& a, float& b) const {
-    const float2 v = pd[c]; a = v.x; b = v.y;
-  }
-  __device__ __forceinline__ void put_q(int c, float x, float y, float z) {
-    q[c] = make_float4(x, y, z, 0.f);
-  }
-  __device__ __forceinline__ void get_q(int c, float& x, float& y, float& z) const {
-    const float4 v = q[c]; x = v.x; y = v.y; z = v.z;
-  }
+template <typename T> struct Pair2;
+template <> struct Pair2<double> { using type = double2; };
+template <> struct Pair2<float> { using type = float2; };
+template <typename T, int CELLS> struct K1Buf {
+  typename Pair2<T>::type pd[CELLS];   // z-combinations of phi^n at a flux plane:
+                                       //   (phi(z-1)+phi(z+1)) + 4 phi(z),  phi(z+1) - phi(z-1)
+  T dv[8][CELLS];                      // divergence contributions sent to the 8 in-plane neighbours
 };
 
 // Software pipeline of iteration j (all inside one barrier interval):
 //   (a) ring-2 threads publish the z-combinations of phi^n for plane j+1,
 //   (b) ring-1 threads turn the combinations of plane j (published one iteration ago) into the
-//       flux Q(j) and publish the z-combinations of Q for plane j-1,
-//   (c) main threads turn the combinations of Q for plane j-2 into phi^{n+1}(j-2).
+//       flux Q(j), combine Q(j-2), Q(j-1), Q(j) along z (Eq. 18 is separable) and SCATTER the
+//       in-plane part of div Q for plane j-1: the neighbour in direction d receives
+//       w(dx) w(dy) (Z - dx X - dy Y), with integer weights (1,4,1) and the factor 1/216 deferred,
+//   (c) main threads sum the 8 contributions published one iteration ago for plane j-2, add
+//       their own 16 Z, and write phi^{n+1}(j-2).
 // Global loads (phi two planes ahead, u one plane ahead) are issued one iteration before use.
-template <typename T, int TX, int TY, int MINB>
+template <typename T, int TX, int TY, int MINB, bool WALLS>
 __global__ void __launch_bounds__((TileMap<TX, TY, 2>::NTHREADS), MINB)
 k_allen_cahn_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ phin, int zchunk) {
   using M = TileMap<TX, TY, 2>;
-  __shared__ K1Buf<T, M::CELLS> sm[2];
+  using P2 = typename Pair2<T>::type;
+  extern __shared__ __align__(16) unsigned char k1_smem_raw[];
+  K1Buf<T, M::CELLS>* sm = reinterpret_cast<K1Buf<T, M::CELLS>*>(k1_smem_raw);
 
   const int tid = threadIdx.x;
   int lx, ly;
@@ -289,39 +272,46 @@ k_allen_cahn_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ phin
                      gx <= P.nx && gy >= -1 && gy <= P.ny;
   const bool is_out = tid < M::NMAIN && gx < P.nx && gy < P.ny;
   int kx = 0, ky = 0;
-  const int sx = ghost_index(min(max(gx, -2), P.nx + 1), P.nx, P.bcx, kx);
-  const int sy = ghost_index(min(max(gy, -2), P.ny + 1), P.ny, P.bcy, ky);
+  const int sx = ghost_index(min(max(gx, -2), P.nx + 1), P.nx, WALLS ? P.bcx : 0, kx);
+  const int sy = ghost_index(min(max(gy, -2), P.ny + 1), P.ny, WALLS ? P.bcy : 0, ky);
   const int col = sx + P.nx * sy;
   const int plane = P.nx * P.ny;
-  const T* phi = S + F_PHI * P.N;
+  const T* phic = S + F_PHI * P.N + col;
+  const int bcz = WALLS ? P.bcz : 0, nz = P.nz;
 
-  auto load_phi = [&](int z) {
-    int kz;
-    return __ldg(phi + col + (long long)plane * ghost_index(z, P.nz, P.bcz, kz));
+  // plane index of z in [-nz, 2nz): periodic wrap or even mirror (R19); kz = crossed a wall
+  auto zsrc = [&](int z, int& kz) {
+    kz = 0;
+    if (z < 0) { if (bcz) { kz = 1; return -1 - z; } return z + nz; }
+    if (z >= nz) { if (bcz) { kz = 1; return 2 * nz - 1 - z; } return z - nz; }
+    return z;
   };
-  // phi u at plane z with velocity-like ghosts (sign flips once per wall crossed, R19)
-  auto load_u = [&](int z, T& ux, T& uy, T& uz) {
+  auto load_phi = [&](int z) { int kz; return __ldg(phic + plane * zsrc(z, kz)); };
+  // u at plane z; velocity-like ghosts change sign once per wall crossed (R19): the sign is
+  // returned and applied where the value is consumed, so the load stays a prefetch
+  auto load_uz = [&](int z, T& ux, T& uy, T& uz, bool& neg) {
     int kz;
-    const int jz = ghost_index(z, P.nz, P.bcz, kz);
-    tslb::load_u(S, P.N, col + (long long)plane * jz, ux, uy, uz);
-    if ((kx + ky + kz) & 1) { ux = -ux; uy = -uy; uz = -uz; }
+    const int jz = zsrc(z, kz);
+    load_u(S, P.N, col + plane * jz, ux, uy, uz);
+    neg = WALLS && ((kx + ky + kz) & 1);
   };
 
-  // phi^n of the own column at planes j, j+1, j+2 (after the shift inside iteration j)
-  T f0 = 0, f1 = 0, f2 = 0, fn = 0;
+  T f0 = 0, f1 = 0, f2 = 0, fn = 0;              // phi^n of the own column at planes j, j+1, j+2
   T un[3] = {};                                  // prefetched u of the next flux plane
+  bool un_neg = false;
   T Qa[3] = {}, Qb[3] = {};                      // Q at planes j-2, j-1
   T sw1 = 0, sw2 = 0, ph1 = 0, ph2 = 0;          // smoothing of pz and phi at planes j-1, j-2
+  T zz1 = 0;                                     // own Z of plane j-2 (computed in iteration j-1)
 
-  // prologue: publish plane z0-1, prefetch what iteration z0-1 consumes
-  if (ring2) {
+  if (ring2) {                                   // prologue: publish plane z0-1
     const T a = load_phi(z0 - 2);
     f1 = load_phi(z0 - 1);
     f2 = load_phi(z0);
     fn = load_phi(z0 + 1);
-    sm[0].put_pd(c, fma(T(4), f1, a + f2), f2 - a);
+    P2 v; v.x = fma(T(4), f1, a + f2); v.y = f2 - a;
+    sm[0].pd[c] = v;
   }
-  if (ring1) load_u(z0 - 1, un[0], un[1], un[2]);
+  if (ring1) load_uz(z0 - 1, un[0], un[1], un[2], un_neg);
   __syncthreads();
 
   for (int j = z0 - 1; j <= z1 + 1; ++j) {
@@ -329,57 +319,57 @@ k_allen_cahn_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ phin
     // (a) publish plane j+1
     f0 = f1; f1 = f2; f2 = fn;
     if (ring2 && j + 1 <= z1) {
-      sm[b ^ 1].put_pd(c, fma(T(4), f1, f0 + f2), f2 - f0);
+      P2 v; v.x = fma(T(4), f1, f0 + f2); v.y = f2 - f0;
+      sm[b ^ 1].pd[c] = v;
       if (j + 3 <= z1 + 1) fn = load_phi(j + 3);
     }
-    // (b) flux of plane j, z-combinations of Q for plane j-1
-    T sw0 = 0;
+    // (b) flux of plane j, scatter of div Q for plane j-1
+    T sw0 = 0, zz0 = 0;
     if (ring1 && j <= z1) {
+      const T fs = un_neg ? -f0 : f0;              // phi u with the ghost sign of u
       const T u0 = un[0], u1 = un[1], u2 = un[2];
-      if (j + 1 <= z1) load_u(j + 1, un[0], un[1], un[2]);
+      if (j + 1 <= z1) load_uz(j + 1, un[0], un[1], un[2], un_neg);
       T rs[3], rd[3], zs[3];
 #pragma unroll
       for (int r = 0; r < 3; ++r) {
         const int cc = c + (r - 1) * M::W;
-        T am, a0, ap, bm, b0, bp;
-        sm[b].get_pd(cc - 1, am, bm);
-        sm[b].get_pd(cc, a0, b0);
-        sm[b].get_pd(cc + 1, ap, bp);
-        rs[r] = fma(T(4), a0, am + ap);
-        rd[r] = ap - am;
-        zs[r] = fma(T(4), b0, bm + bp);
+        const P2 m = sm[b].pd[cc - 1], o = sm[b].pd[cc], p = sm[b].pd[cc + 1];
+        rs[r] = fma(T(4), o.x, m.x + p.x);
+        rd[r] = p.x - m.x;
+        zs[r] = fma(T(4), o.y, m.y + p.y);
       }
       sw0 = fma(T(4), rs[1], rs[0] + rs[2]);
       const T g0 = fma(T(4), rd[1], rd[0] + rd[2]) * T(3.0 / 216.0);
       const T g1 = (rs[2] - rs[0]) * T(3.0 / 216.0);
       const T g2 = fma(T(4), zs[1], zs[0] + zs[2]) * T(3.0 / 216.0);
       const T s = P.kappa_ac * f0 * (T(1) - f0) * rsqrt_t(g0 * g0 + g1 * g1 + g2 * g2 + T(1e-24));
-      const T Qc0 = fma(f0, u0, s * g0), Qc1 = fma(f0, u1, s * g1), Qc2 = fma(f0, u2, s * g2);
-      sm[b].put_q(c, fma(T(4), Qb[0], Qa[0] + Qc0), fma(T(4), Qb[1], Qa[1] + Qc1), Qc2 - Qa[2]);
+      const T Qc0 = fma(fs, u0, s * g0), Qc1 = fma(fs, u1, s * g1), Qc2 = fma(fs, u2, s * g2);
+      const T X = fma(T(4), Qb[0], Qa[0] + Qc0), Y = fma(T(4), Qb[1], Qa[1] + Qc1);
+      zz0 = Qc2 - Qa[2];
       Qa[0] = Qb[0]; Qa[1] = Qb[1]; Qa[2] = Qb[2];
       Qb[0] = Qc0; Qb[1] = Qc1; Qb[2] = Qc2;
+      // direction d = (dx,dy): slot order (-1,-1) (0,-1) (1,-1) (-1,0) (1,0) (-1,1) (0,1) (1,1)
+      const T zpx = zz0 + X, zmx = zz0 - X;
+      sm[b].dv[0][c] = zpx + Y;                    // d = (-1,-1):  Z + X + Y
+      sm[b].dv[1][c] = T(4) * (zz0 + Y);           // d = ( 0,-1):  4 (Z + Y)
+      sm[b].dv[2][c] = zmx + Y;                    // d = ( 1,-1):  Z - X + Y
+      sm[b].dv[3][c] = T(4) * zpx;                 // d = (-1, 0):  4 (Z + X)
+      sm[b].dv[4][c] = T(4) * zmx;                 // d = ( 1, 0):  4 (Z - X)
+      sm[b].dv[5][c] = zpx - Y;                    // d = (-1, 1):  Z + X - Y
+      sm[b].dv[6][c] = T(4) * (zz0 - Y);           // d = ( 0, 1):  4 (Z - Y)
+      sm[b].dv[7][c] = zmx - Y;                    // d = ( 1, 1):  Z - X - Y
     }
-    // (c) output plane k = j-2 from the combinations published one iteration ago
+    // (c) output plane k = j-2: arrivals from the source at -d, published one iteration ago
     const int k = j - 2;
     if (is_out && k >= z0) {
-      T rx[3], ry[3], rz[3];
-#pragma unroll
-      for (int r = 0; r < 3; ++r) {
-        const int cc = c + (r - 1) * M::W;
-        T xm, ym, zm, x0, y0, z0_, xp, yp, zp;
-        sm[b ^ 1].get_q(cc - 1, xm, ym, zm);
-        sm[b ^ 1].get_q(cc, x0, y0, z0_);
-        sm[b ^ 1].get_q(cc + 1, xp, yp, zp);
-        rx[r] = xp - xm;
-        ry[r] = fma(T(4), y0, ym + yp);
-        rz[r] = fma(T(4), z0_, zm + zp);
-      }
-      // div Q = 3/216 [ (1,4,1)_y (x) d_x X + d_y (x) (1,4,1)_x Y + (1,4,1)^2 Z ]
-      const T div = fma(T(4), rx[1], rx[0] + rx[2]) + (ry[2] - ry[0]) + fma(T(4), rz[1], rz[0] + rz[2]);
+      const K1Buf<T, M::CELLS>& r = sm[b ^ 1];
+      T div = T(16) * zz1;
+      div += (r.dv[0][c + M::W + 1] + r.dv[7][c - M::W - 1]) + (r.dv[2][c + M::W - 1] + r.dv[5][c - M::W + 1]);
+      div += (r.dv[1][c + M::W] + r.dv[6][c - M::W]) + (r.dv[3][c + 1] + r.dv[4][c - 1]);
       const T lap = fma(T(6.0 / 216.0), sw2, T(-6) * ph2);
-      phin[gx + P.nx * gy + (long long)plane * k] = ph2 - T(3.0 / 216.0) * div + P.mob * lap;
+      phin[gx + P.nx * gy + plane * k] = ph2 - T(3.0 / 216.0) * div + P.mob * lap;
     }
-    sw2 = sw1; sw1 = sw0; ph2 = ph1; ph1 = f0;
+    sw2 = sw1; sw1 = sw0; ph2 = ph1; ph1 = f0; zz1 = zz0;
     __syncthreads();
   }
 }
