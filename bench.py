@@ -221,30 +221,54 @@ def measure_e2e(cfg, precision, args, device, flags):
                 note="host->device init + K steps + device->host read of rho,p,u,phi, wall clock")
 
 
+class Ranks:
+    """One process per GPU (torchrun env).  Replicas only: the data path has no collective; the
+    only communication is the timing protocol (barrier, max of the device time over ranks)."""
+
+    def __init__(self, backend):
+        import torch
+        import torch.distributed as dist
+        self.torch, self.dist = torch, dist
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        self.backend = backend
+        self.device = f"cuda:{self.local}" if backend == "nccl" else "cpu"
+        if self.world > 1:
+            kw = {"device_id": torch.device(self.device)} if backend == "nccl" else {}
+            dist.init_process_group(backend, **kw)
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+
+    def max(self, x):
+        if self.world == 1:
+            return x
+        t = self.torch.tensor([x], dtype=self.torch.float64, device=self.device)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def close(self):
+        if self.world > 1:
+            self.dist.destroy_process_group()
+
+
+def whole_job_glups(nodes, steps, ms_max, world):
+    """Aggregate over all replicas: every rank advanced `nodes` nodes by `steps` steps in at most
+    ms_max milliseconds (max over ranks)."""
+    return world * nodes * steps / (ms_max * 1e-3) / 1e9
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
     import torch
-    import torch.distributed as dist
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    device = f"cuda:{local}"
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(device))
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-
-    def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    ranks = Ranks("nccl")
+    world, rank, device = ranks.world, ranks.rank, ranks.device
+    torch.cuda.set_device(ranks.local)
+    barrier, max_over_ranks = ranks.barrier, ranks.max
 
     flags = (1 if args.naive else 0) | (2 if args.generic else 0) | (args.variant << 8) | (args.k1variant << 16)
     cfg = make_workload(args.size)
@@ -256,7 +280,7 @@ def main():
         r = measure(cfg, prec, args, device, flags, barrier)
         r["ms"] = max_over_ranks(r["ms"])
         es = 8 if prec == "f64" else 4
-        r["glups"] = world * n * args.steps / (r["ms"] * 1e-3) / 1e9
+        r["glups"] = whole_job_glups(n, args.steps, r["ms"], world)
         # dominant kernel and its roofline: algorithmic bytes of the
         # whole update, 28 s per node, charged to the dominant kernel's own duration only when
         # the step is a single kernel; for a split step each kernel is charged its own planes.
@@ -308,8 +332,7 @@ def main():
                           "roofline": o["roofline"], "clocks": o["clocks"],
                           "gpu_launches": o["launches"], "finite": o["finite"]}
         print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    ranks.close()
 
 
 if __name__ == "__main__":

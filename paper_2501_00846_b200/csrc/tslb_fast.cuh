@@ -152,13 +152,49 @@ __device__ __forceinline__ Red6<T> reduce6(const T (&v)[3][3]) {   // v[cx+1][cy
   return r;
 }
 
-template <typename T, int TX, int TY, int MINB, bool PREFETCH>
+// ---- cp.async staging of the next source planes (memory pipeline without registers) ---------
+// The kernel is bound by global-memory latency unless several planes per SM are in flight
+// (profiles/r1_ablation.md), and fp64 has no registers to spare for a deeper prefetch.  Each
+// thread therefore copies the 14 scalars of ITS OWN node for plane j+NSTAGE straight into a
+// private shared-memory slot (cp.async, no register staging) and picks them up NSTAGE iterations
+// later; only cp.async.wait_group is needed, no block barrier, because nobody else reads the slot.
+template <typename T, int CELLS>
+struct StageBuf {
+  typename VecOf<T>::type vec[12 / VecOf<T>::W][CELLS];
+  T az[CELLS];
+  T ph[CELLS];
+};
+__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(dst)), "l"(src));
+}
+__device__ __forceinline__ void cp_async_small(double* dst, const double* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(dst)), "l"(src));
+}
+__device__ __forceinline__ void cp_async_small(float* dst, const float* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(dst)), "l"(src));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+// ABL != 0 : timing ablations (wrong results on purpose; never selected in production)
+//   bit mask: 1 no shared-memory reads, 2 no closing arithmetic, 4 no global stores,
+//   8 no global loads, 16 no source arithmetic (main warps), 32 no shared-memory writes
+// NSTAGE > 0 : cp.async staging NSTAGE planes ahead (PREFETCH is then ignored)
+template <typename T, int TX, int TY, int MINB, bool PREFETCH, int ABL = 0, int NSTAGE = 0>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
 k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D, int zchunk) {
   using M = TileMap<TX, TY, 1>;
   using SM = K2FastSmem<T, M::CELLS>;
+  using STG = StageBuf<T, M::CELLS>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
+  STG* stg = reinterpret_cast<STG*>(smem_raw + sizeof(SM));      // NSTAGE slots (if any)
+  constexpr bool REGPF = PREFETCH && NSTAGE == 0;
 
   const int tid = threadIdx.x;
   int lx, ly;
@@ -175,6 +211,34 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   const int col = in_ring ? sx + P.nx * sy : 0;
   const T* phin = D + F_PHI * P.N;
 
+  // cp.async pipeline: one commit group per plane, issued by every thread (possibly empty)
+  auto stage_issue = [&](int j, int slot) {
+    if (NSTAGE > 0) {
+      if (in_ring && j <= z1) {
+        using V = typename VecOf<T>::type;
+        const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
+        const int s = col + plane * jz;
+        const V* g = reinterpret_cast<const V*>(S);
+#pragma unroll
+        for (int k = 0; k < 12 / VecOf<T>::W; ++k) cp_async16(&stg[slot].vec[k][c], g + k * P.N + s);
+        cp_async_small(&stg[slot].az[c], S + 12 * P.N + s);
+        cp_async_small(&stg[slot].ph[c], phin + s);
+      }
+      cp_async_commit();
+    }
+  };
+  auto stage_take = [&](int slot, T (&m)[13], T& ph) {
+    constexpr int W = VecOf<T>::W;
+#pragma unroll
+    for (int k = 0; k < 12 / W; ++k) unpack(stg[slot].vec[k][c], &m[k * W]);
+    m[12] = stg[slot].az[c];
+    ph = stg[slot].ph[c];
+  };
+  if (NSTAGE > 0) {
+#pragma unroll
+    for (int d = 0; d < NSTAGE; ++d) stage_issue(z0 - 1 + d, d);
+  }
+
   // Register pipeline along z.  Two slots alternate roles every plane ("A" = destination plane
   // j-1, completed in iteration j; "B" = destination plane j), so the marching loop is unrolled
   // by two and no register is moved to shift the pipeline.
@@ -185,18 +249,60 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   auto load_plane = [&](int j, T (&m)[13], T& ph) {
     const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
     const int s = col + plane * jz;
-    load13(S, P.N, s, m);
-    ph = __ldg(phin + s);
+    if (ABL & 8) {
+#pragma unroll
+      for (int f = 0; f < 13; ++f) m[f] = T(1e-3) * T(f + (s & 7));
+      ph = T(0.5);
+    } else {
+      load13(S, P.N, s, m);
+      ph = __ldg(phin + s);
+    }
   };
-  if (PREFETCH && in_ring) load_plane(z0 - 1, nxt, nxt_phi);
+  // ---- halo warps: sources only.  They have no receive phase to hide the memory latency of
+  // the next plane behind, and every main warp waits for them at the barrier, so they prefetch
+  // TWO planes ahead (registers are plentiful here: no accumulators).
+  if (REGPF && tid >= M::NMAIN) {
+    T pa[13], pb[13], fa = 0, fb = 0;
+    if (in_ring) {
+      load_plane(z0 - 1, pa, fa);
+      load_plane(z0, pb, fb);
+    }
+    for (int j = z0 - 1; j <= z1; ++j) {
+      ExBuf<T, M::CELLS>& xb = sm.buf[(j - z0 + 1) & 1];
+      ph_m = ph_0; ph_0 = ph_p;
+      if (in_ring) {
+        T cur[13];
+#pragma unroll
+        for (int f = 0; f < 13; ++f) { cur[f] = pa[f]; pa[f] = pb[f]; }
+        ph_p = fa; fa = fb;
+        if (j + 2 <= z1) load_plane(j + 2, pb, fb);
+        const Coef<T> cf = coef_from13(cur);
+        SrcFields<T> sf;
+        source_fields(cf, sf);
+#pragma unroll
+        for (int q = 0; q < 9; ++q) {
+          const int cx = q % 3 - 1, cy = q / 3 - 1;
+          if (cx == 0 && cy == 0) continue;
+          xb.put(dir_slot(cx, cy), c, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
+        }
+        xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
+      }
+      __syncthreads();
+    }
+    return;
+  }
+  if (REGPF && in_ring) load_plane(z0 - 1, nxt, nxt_phi);
 
-  auto body = [&](const int j, ExBuf<T, M::CELLS>& xb, T (&aA)[6], T (&aB)[6], T (&zA)[3],
-                  T (&zB)[3], const T (&uPrev)[3], T (&uCur)[3]) {
+  auto body = [&](const int j, const int slot, ExBuf<T, M::CELLS>& xb, T (&aA)[6], T (&aB)[6],
+                  T (&zA)[3], T (&zB)[3], const T (&uPrev)[3], T (&uCur)[3]) {
     T ownE = 0, ownO = 0, ownQ = 0;
     ph_m = ph_0; ph_0 = ph_p;
     if (in_ring) {
       T cur[13];
-      if (PREFETCH) {
+      if (NSTAGE > 0) {
+        cp_async_wait<(NSTAGE > 0 ? NSTAGE - 1 : 0)>();        // the group of plane j has landed
+        stage_take(slot, cur, ph_p);
+      } else if (REGPF) {
 #pragma unroll
         for (int f = 0; f < 13; ++f) cur[f] = nxt[f];
         ph_p = nxt_phi;
@@ -204,20 +310,26 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         load_plane(j, cur, ph_p);
       }
       uCur[0] = cur[F_UX]; uCur[1] = cur[F_UY]; uCur[2] = cur[F_UZ];
-      const Coef<T> cf = coef_from13(cur);
       SrcFields<T> sf;
-      source_fields(cf, sf);
+      if (ABL & 16) {
+#pragma unroll
+        for (int a = 0; a < 9; ++a) { sf.E[a / 3][a % 3] = cur[a]; sf.O[a / 3][a % 3] = cur[a + 2]; sf.Q[a / 3][a % 3] = cur[a + 4]; }
+      } else {
+        const Coef<T> cf = coef_from13(cur);
+        source_fields(cf, sf);
+      }
       ownE = sf.E[1][1]; ownO = sf.O[1][1]; ownQ = sf.Q[1][1];
 #pragma unroll
       for (int q = 0; q < 9; ++q) {
         const int cx = q % 3 - 1, cy = q / 3 - 1;
         if (cx == 0 && cy == 0) continue;
-        xb.put(dir_slot(cx, cy), c, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
+        if (!(ABL & 32) || cx + cy == 2) xb.put(dir_slot(cx, cy), c, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
       }
       xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
     }
+    stage_issue(j + NSTAGE, slot);             // refill the slot just consumed (no-op if NSTAGE = 0)
     __syncthreads();
-    if (PREFETCH && in_ring && j < z1) load_plane(j + 1, nxt, nxt_phi);
+    if (REGPF && in_ring && j < z1) load_plane(j + 1, nxt, nxt_phi);
 
     if (is_out) {
       Red6<T> rE, rO, rQ;
@@ -228,6 +340,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         for (int q = 0; q < 9; ++q) {
           const int cx = q % 3 - 1, cy = q / 3 - 1;
           if (cx == 0 && cy == 0) continue;
+          if ((ABL & 1) && q != 8) { vE[cx + 1][cy + 1] = ownE * T(q); vO[cx + 1][cy + 1] = ownO * T(q); continue; }
           xb.get_eo(dir_slot(cx, cy), c - cy * M::W - cx, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
         }
         rE = reduce6(vE);
@@ -241,6 +354,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         for (int q = 0; q < 9; ++q) {
           const int cx = q % 3 - 1, cy = q / 3 - 1;
           if (cx == 0 && cy == 0) continue;
+          if ((ABL & 1) && q != 8) { vQ[cx + 1][cy + 1] = ownQ * T(q); continue; }
           xb.get_q(dir_slot(cx, cy), c - cy * M::W - cx, vQ[cx + 1][cy + 1]);
         }
         rQ = reduce6(vQ);
@@ -272,9 +386,12 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         for (int r = 0; r < 3; ++r) {
           const int cc = c + (r - 1) * M::W;
           T am, a0, ap, bm, b0, bp;
+          if (ABL & 1) { am = a0 = ap = ph_0 * T(r); bm = b0 = bp = ph_p; }
+          else {
           xb.get_pd(cc - 1, am, bm);
           xb.get_pd(cc, a0, b0);
           xb.get_pd(cc + 1, ap, bp);
+          }
           rs[r] = fma(T(4), a0, am + ap);
           rd[r] = ap - am;
           zs[r] = fma(T(4), b0, bm + bp);
@@ -284,8 +401,10 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         const T gy_ = (rs[2] - rs[0]) * T(3.0 / 216.0);
         const T gz_ = fma(T(4), zs[1], zs[0] + zs[2]) * T(3.0 / 216.0);
         const T lap = fma(T(6.0 / 216.0), sw, T(-6) * ph_0);
-        const NodeOut<T> out = close_node(P, m, ph_0, gx_, gy_, gz_, lap, uPrev[0], uPrev[1], uPrev[2]);
-        store_out(D, P.N, gx + P.nx * gy + plane * k, out);
+        NodeOut<T> out;
+        if (ABL & 2) { out.p = m.p + lap; out.ux = m.mx + gx_; out.uy = m.my + gy_; out.uz = m.mz + gz_; out.axx = m.xx; out.ayy = m.yy; out.azz = m.zz; out.axy = m.xy; out.axz = m.xz; out.ayz = m.yz; out.ax = uPrev[0]; out.ay = uPrev[1]; out.az = uPrev[2]; }
+        else out = close_node(P, m, ph_0, gx_, gy_, gz_, lap, uPrev[0], uPrev[1], uPrev[2]);
+        if (!(ABL & 4) || out.p == T(123.456)) store_out(D, P.N, gx + P.nx * gy + plane * k, out);
       }
       // slot A is free now: it becomes the accumulator of destination plane j+1
 #pragma unroll
@@ -295,10 +414,17 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
     }
   };
 
+  int slot = 0;                                 // staging slot of plane j: (j - z0 + 1) % NSTAGE
+  auto next_slot = [&]() { if (NSTAGE > 1) slot = (slot + 1 == NSTAGE) ? 0 : slot + 1; };
   for (int j = z0 - 1; j <= z1; j += 2) {
-    body(j, sm.buf[0], acc0, acc1, zo0, zo1, u0, u1);
-    if (j + 1 <= z1) body(j + 1, sm.buf[1], acc1, acc0, zo1, zo0, u1, u0);
+    body(j, slot, sm.buf[0], acc0, acc1, zo0, zo1, u0, u1);
+    next_slot();
+    if (j + 1 <= z1) {
+      body(j + 1, slot, sm.buf[1], acc1, acc0, zo1, zo0, u1, u0);
+      next_slot();
+    }
   }
+  if (NSTAGE > 0) cp_async_wait<0>();
 }
 
 }  // namespace tslb

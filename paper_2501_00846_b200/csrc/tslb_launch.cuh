@@ -1,6 +1,7 @@
 // tslb_launch.cuh -- launch of one time step: kernel selection, grid sizing, attributes.
 #pragma once
 #include "tslb_fast.cuh"
+#include "tslb_stag.cuh"
 #include "tslb_tiled.cuh"
 
 namespace tslb {
@@ -16,11 +17,28 @@ inline cudaError_t prepare(K kernel, size_t smem) {
                               cudaSharedmemCarveoutMaxShared);
 }
 
-template <typename T, int TY, int MINB, bool PREFETCH>
+template <typename T, int TY, int MINB, bool PREFETCH, int ABL = 0, int NSTAGE = 0>
 cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream) {
   constexpr int TX = 32;
   using M = TileMap<TX, TY, 1>;
-  auto kernel = k_stream_collide_fast<T, TX, TY, MINB, PREFETCH>;
+  auto kernel = k_stream_collide_fast<T, TX, TY, MINB, PREFETCH, ABL, NSTAGE>;
+  const size_t smem = sizeof(K2FastSmem<T, M::CELLS>) + NSTAGE * sizeof(StageBuf<T, M::CELLS>);
+  static bool ready = false;
+  if (!ready) {
+    cudaError_t e = prepare(kernel, smem);
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
+  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, ZCHUNK);
+  return cudaGetLastError();
+}
+
+template <typename T, int TY, int MINB>
+cudaError_t launch_stag(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream) {
+  constexpr int TX = 32;
+  using M = TileMap<TX, TY, 1>;
+  auto kernel = k_stream_collide_stag<T, TX, TY, MINB>;
   const size_t smem = sizeof(K2FastSmem<T, M::CELLS>);
   static bool ready = false;
   if (!ready) {
@@ -96,11 +114,25 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, cudaStream_t stre
     switch (variant) {
       default:   // production choice: fp64 one block/SM, fp32 two blocks/SM
       case 0:
-        e = sizeof(T) == 8 ? launch_fast<T, 8, 1, true>(P, S, D, stream)
-                           : launch_fast<T, 8, 2, false>(P, S, D, stream);
+        e = sizeof(T) == 8 ? launch_fast<T, 8, 1, false, 0, 1>(P, S, D, stream)
+                           : launch_fast<T, 8, 2, false, 0, 1>(P, S, D, stream);
         break;
       case 6: e = launch_fast<T, 8, 1, false>(P, S, D, stream); break;
       case 7: e = launch_fast<T, 4, 2, false>(P, S, D, stream); break;
+      case 21: e = launch_fast<T, 8, 1, true, 4>(P, S, D, stream); break;    // timing ablations
+      case 22: e = launch_fast<T, 8, 1, true, 8>(P, S, D, stream); break;
+      case 23: e = launch_fast<T, 8, 1, true, 12>(P, S, D, stream); break;
+      case 24: e = launch_fast<T, 8, 1, true, 16>(P, S, D, stream); break;
+      case 25: e = launch_fast<T, 8, 1, true, 1 + 2 + 32>(P, S, D, stream); break;
+      case 26: e = launch_fast<T, 8, 1, true, 1 + 2 + 16 + 32>(P, S, D, stream); break;
+      case 27: e = launch_fast<T, 8, 1, true, 1 + 2 + 4 + 16 + 32>(P, S, D, stream); break;
+      case 28: e = launch_fast<T, 8, 1, true, 63>(P, S, D, stream); break;
+      case 30: e = launch_fast<T, 8, 1, false, 0, 1>(P, S, D, stream); break;   // cp.async staging
+      case 31: e = launch_fast<T, 8, 1, false, 0, 2>(P, S, D, stream); break;
+      case 32: e = launch_fast<T, 8, 2, false, 0, 1>(P, S, D, stream); break;
+      case 10: e = launch_stag<T, 8, 1>(P, S, D, stream); break;
+      case 11: e = launch_stag<T, 8, 2>(P, S, D, stream); break;
+      case 12: e = launch_stag<T, 4, 2>(P, S, D, stream); break;
       case 8: e = launch_fast<T, 4, 2, true>(P, S, D, stream); break;
       case 9: e = launch_fast<T, 4, 3, false>(P, S, D, stream); break;
       case 1: e = launch_fast<T, 8, 1, true>(P, S, D, stream); break;

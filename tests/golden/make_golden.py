@@ -1,0 +1,95 @@
+#!/usr/bin/env python
+"""Write long-horizon expected values with the CPU ORACLE ONLY (never the CUDA path).
+
+Usage:  python tests/golden/make_golden.py [case ...]      (no argument = every case)
+
+For each case the oracle runs the seeded input of paper_2501_00846_b200.inputs for the
+config's full step count and stores, at the checkpoints {1, 10, 100, 1000, ..., final}:
+  * rho, p, u, phi at NSAMPLE seeded node positions (element-by-element parity on samples),
+  * per-field max|.| over the whole lattice (the denominators of the parity norm),
+  * the diagnostics sum(phi), sum(p*), and for droplets the Laplace ratio of pin P9.
+Files: tests/golden/<case>.npz (a few hundred kB each).  tests/test_golden_gpu.py replays the
+same inputs through the C ABI and compares.
+
+Cases (BASELINE.json configs):
+  laplace128_R12   configs[1], 128^3, R = 12, 2000 steps               (~1.5 h on 8 cores)
+  collision64      configs[3] scaled to 64^3 (R = 6, same We/Re/ratios), 1500 steps
+  bubble32x32x64   configs[2] scaled to 32x32x64 (R = 4, walls in z), 2000 steps
+  droplet32        configs[0], 32^3, R = 8, 200 steps
+"""
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+
+from oracle import tslb_ref as R                      # noqa: E402
+from paper_2501_00846_b200 import inputs as I          # noqa: E402
+
+NSAMPLE = 2048
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def cases():
+    return {
+        "droplet32": (lambda: I.static_droplet(32, 8.0, seed=1), [1, 10, 100, 200]),
+        "collision64": (lambda: I.head_on_collision(n=64, radius=6.0, half_sep=10.0),
+                        [1, 10, 100, 1000, 1500]),
+        "bubble32x32x64": (lambda: I.rising_bubble(nx=32, ny=32, nz=64, radius=4.0, height=10.0),
+                           [1, 10, 100, 1000, 2000]),
+        "laplace128_R12": (lambda: I.static_droplet(128, 12.0, seed=12), [1, 10, 100, 1000, 2000]),
+    }
+
+
+def sample_index(shape, seed=12345):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    n = int(np.prod(shape))
+    return np.sort(rng.choice(n, size=min(NSAMPLE, n), replace=False))
+
+
+def laplace_ratio(p, phi, sigma):
+    inside, outside = phi > 0.99, phi < 0.01
+    if not inside.any() or not outside.any():
+        return np.nan
+    dp = p[inside].mean() - p[outside].mean()
+    r_eff = (3.0 * phi.sum() / (4.0 * np.pi)) ** (1.0 / 3.0)
+    return dp * r_eff / (2.0 * sigma)
+
+
+def run(name):
+    make, checkpoints = cases()[name]
+    cfg = make()
+    nz, ny, nx = cfg["shape"]
+    idx = sample_index(cfg["shape"])
+    sim = R.RefSim(nx, ny, nz, R.make_params(**cfg["params"]))
+    sim.init(cfg["phi"], cfg["u"])
+    out = {"checkpoints": np.array(checkpoints), "sample_index": idx,
+           "shape": np.array(cfg["shape"])}
+    done, t0 = 0, time.time()
+    for cp in checkpoints:
+        sim.step(cp - done)
+        done = cp
+        rho, p, u, phi = sim.get()
+        ps = sim.get_state()[0]
+        out[f"rho_{cp}"] = rho.ravel()[idx]
+        out[f"p_{cp}"] = p.ravel()[idx]
+        out[f"phi_{cp}"] = phi.ravel()[idx]
+        out[f"u_{cp}"] = u.reshape(3, -1)[:, idx]
+        out[f"max_{cp}"] = np.array([np.abs(rho).max(), np.abs(p).max(), np.abs(u).max(),
+                                     np.abs(phi).max()])
+        out[f"diag_{cp}"] = np.array([phi.sum(), ps.sum(),
+                                      laplace_ratio(p, phi, cfg["params"]["sigma"]),
+                                      float(np.isfinite(u).all())])
+        print(f"{name}: step {cp} done after {time.time() - t0:.0f} s, max|u| = "
+              f"{np.abs(u).max():.3e}, sum(phi) drift = {phi.sum() / cfg['phi'].sum() - 1:.1e}",
+              flush=True)
+    sim.close()
+    np.savez_compressed(os.path.join(HERE, name + ".npz"), **out)
+
+
+if __name__ == "__main__":
+    for nm in (sys.argv[1:] or list(cases())):
+        run(nm)

@@ -1,0 +1,66 @@
+"""Long-horizon parity: the CUDA path against expected values written by the CPU oracle
+(tests/golden/make_golden.py, which calls only oracle/).  Error is reported against step count
+(SURVEY.md 7.3-4); the bar is BASELINE.json's at every checkpoint."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2501_00846_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+CASES = {
+    "droplet32": lambda: I.static_droplet(32, 8.0, seed=1),
+    "collision64": lambda: I.head_on_collision(n=64, radius=6.0, half_sep=10.0),
+    "bubble32x32x64": lambda: I.rising_bubble(nx=32, ny=32, nz=64, radius=4.0, height=10.0),
+    "laplace128_R12": lambda: I.static_droplet(128, 12.0, seed=12),
+}
+
+
+def _errors(g, gold, cp, idx):
+    mx = gold[f"max_{cp}"]
+    out = {}
+    for k, (name, den) in enumerate(zip(("rho", "p", "u", "phi"), mx)):
+        got = g[name].double().reshape(3, -1)[:, idx] if name == "u" else g[name].double().ravel()[idx]
+        out[name] = float(np.abs(got.cpu().numpy() - gold[f"{name}_{cp}"]).max() / den)
+    return out
+
+
+@pytest.mark.parametrize("case", list(CASES))
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_against_golden(case, precision):
+    path = os.path.join(HERE, case + ".npz")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated")
+    import torch
+    from paper_2501_00846_b200 import binding as B
+    gold = np.load(path)
+    cfg = CASES[case]()
+    assert tuple(gold["shape"]) == cfg["shape"]
+    nz, ny, nx = cfg["shape"]
+    idx = torch.as_tensor(gold["sample_index"], device="cuda")
+    s = B.Solver(nx, ny, nz, cfg["params"], precision=precision)
+    s.init(cfg["phi"], cfg["u"])
+    done = 0
+    tol = 1e-10 if precision == "f64" else 1e-4
+    fields = ("rho", "p", "u", "phi") if precision == "f64" else ("u", "phi")
+    worst = {}
+    for cp in gold["checkpoints"]:
+        cp = int(cp)
+        s.step(cp - done)
+        done = cp
+        g = s.get()
+        errs = _errors(g, gold, cp, idx)
+        st = s.get_state()
+        sum_phi = float(g["phi"].double().sum())
+        sum_ps = float(st["pstar"].double().sum())
+        print(f"[{case} {precision}] step {cp}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items())
+              + f" | sum(phi) rel diff {sum_phi / gold[f'diag_{cp}'][0] - 1:.1e}"
+              + f" sum(p*) {sum_ps:.1e} (oracle {gold[f'diag_{cp}'][1]:.1e})")
+        worst[cp] = {k: errs[k] for k in fields}
+        assert bool(torch.isfinite(g["u"]).all())
+    s.close()
+    bad = {cp: e for cp, e in worst.items() if any(not (v <= tol) for v in e.values())}
+    assert not bad, bad
