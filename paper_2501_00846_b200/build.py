@@ -10,7 +10,7 @@ LIB = os.path.join(HERE, "libtslb.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-cudart", "shared", "-shared", "-Xcompiler", "-fPIC",
-              "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
+              "-Xlinker", "-rpath=/usr/local/cuda/lib64", "-diag-suppress", "128"]
 
 
 def sources():

@@ -214,7 +214,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   // cp.async pipeline: one commit group per plane, issued by every thread (possibly empty)
   auto stage_issue = [&](int j, int slot) {
     if (NSTAGE > 0) {
-      if (in_ring && j <= z1) {
+      if (in_ring && j <= z1 && !(ABL & 8)) {
         using V = typename VecOf<T>::type;
         const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
         const int s = col + plane * jz;
@@ -229,6 +229,12 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   };
   auto stage_take = [&](int slot, T (&m)[13], T& ph) {
     constexpr int W = VecOf<T>::W;
+    if (ABL & 8) {
+#pragma unroll
+      for (int f = 0; f < 13; ++f) m[f] = T(1e-3) * T(f + (c & 7));
+      ph = T(0.5);
+      return;
+    }
 #pragma unroll
     for (int k = 0; k < 12 / W; ++k) unpack(stg[slot].vec[k][c], &m[k * W]);
     m[12] = stg[slot].az[c];

@@ -119,14 +119,15 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, cudaStream_t stre
         break;
       case 6: e = launch_fast<T, 8, 1, false>(P, S, D, stream); break;
       case 7: e = launch_fast<T, 4, 2, false>(P, S, D, stream); break;
-      case 21: e = launch_fast<T, 8, 1, true, 4>(P, S, D, stream); break;    // timing ablations
-      case 22: e = launch_fast<T, 8, 1, true, 8>(P, S, D, stream); break;
-      case 23: e = launch_fast<T, 8, 1, true, 12>(P, S, D, stream); break;
-      case 24: e = launch_fast<T, 8, 1, true, 16>(P, S, D, stream); break;
-      case 25: e = launch_fast<T, 8, 1, true, 1 + 2 + 32>(P, S, D, stream); break;
-      case 26: e = launch_fast<T, 8, 1, true, 1 + 2 + 16 + 32>(P, S, D, stream); break;
-      case 27: e = launch_fast<T, 8, 1, true, 1 + 2 + 4 + 16 + 32>(P, S, D, stream); break;
-      case 28: e = launch_fast<T, 8, 1, true, 63>(P, S, D, stream); break;
+      case 21: e = launch_fast<T, 8, 1, false, 4, 1>(P, S, D, stream); break;    // timing ablations
+      case 22: e = launch_fast<T, 8, 1, false, 8, 1>(P, S, D, stream); break;
+      case 23: e = launch_fast<T, 8, 1, false, 12, 1>(P, S, D, stream); break;
+      case 24: e = launch_fast<T, 8, 1, false, 16, 1>(P, S, D, stream); break;
+      case 25: e = launch_fast<T, 8, 1, false, 1 + 2 + 32, 1>(P, S, D, stream); break;
+      case 26: e = launch_fast<T, 8, 1, false, 1 + 2 + 16 + 32, 1>(P, S, D, stream); break;
+      case 27: e = launch_fast<T, 8, 1, false, 1, 1>(P, S, D, stream); break;
+      case 28: e = launch_fast<T, 8, 1, false, 2, 1>(P, S, D, stream); break;
+      case 29: e = launch_fast<T, 8, 1, false, 32, 1>(P, S, D, stream); break;
       case 30: e = launch_fast<T, 8, 1, false, 0, 1>(P, S, D, stream); break;   // cp.async staging
       case 31: e = launch_fast<T, 8, 1, false, 0, 2>(P, S, D, stream); break;
       case 32: e = launch_fast<T, 8, 2, false, 0, 1>(P, S, D, stream); break;
