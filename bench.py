@@ -305,11 +305,11 @@ def main():
         e2e["value"] = world * e2e["value"] if world > 1 else e2e["value"]
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        planes = 16
-        v, dt = time_oracle(cfg, planes, 2)
+        planes, osteps = min(64, cfg["shape"][0]), 8
+        v, dt = time_oracle(cfg, planes, osteps)
         cpu = {"value": v, "unit": "GLUPS", "cores": omp_threads(), "kind": "oracle",
                "sample": f"central {cfg['shape'][2]}x{cfg['shape'][1]}x{planes} slab of the same "
-                         f"input, 2 steps, {dt:.1f} s"}
+                         f"input, {osteps} steps, {dt:.1f} s"}
     if rank == 0:
         line = {"metric": METRIC, "value": head["glups"], "unit": "GLUPS", "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup,

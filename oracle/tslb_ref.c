@@ -10,6 +10,7 @@
 #include <string.h>
 
 #define Q 27
+#define OMP_MIN_NODES 8192   /* below this a pass runs on one thread (team start-up costs more) */
 static const double CS2 = 1.0 / 3.0;     /* R1: cs^2 of D3Q27                       */
 static const double EPS_N = 1e-12;       /* R13: n = grad(phi)/sqrt(|grad(phi)|^2 + eps^2) */
 
@@ -195,7 +196,7 @@ static double div_at(const double *G3, long N, int ix, int iy, int iz, int nx, i
 void tslb_ref_gradient(const double *psi, int nx, int ny, int nz, const int bc[3], double *out3) {
   build_tables();
   long N = (long)nx * ny * nz;
-#pragma omp parallel for
+#pragma omp parallel for if ((long)nx * ny * nz >= OMP_MIN_NODES)
   for (int iz = 0; iz < nz; ++iz)
     for (int iy = 0; iy < ny; ++iy)
       for (int ix = 0; ix < nx; ++ix) {
@@ -208,7 +209,7 @@ void tslb_ref_gradient(const double *psi, int nx, int ny, int nz, const int bc[3
 
 void tslb_ref_laplacian(const double *psi, int nx, int ny, int nz, const int bc[3], double *out) {
   build_tables();
-#pragma omp parallel for
+#pragma omp parallel for if ((long)nx * ny * nz >= OMP_MIN_NODES)
   for (int iz = 0; iz < nz; ++iz)
     for (int iy = 0; iy < ny; ++iy)
       for (int ix = 0; ix < nx; ++ix)
@@ -219,7 +220,7 @@ void tslb_ref_divergence(const double *G3, int nx, int ny, int nz, const int bc[
                          double *out) {
   build_tables();
   long N = (long)nx * ny * nz;
-#pragma omp parallel for
+#pragma omp parallel for if ((long)nx * ny * nz >= OMP_MIN_NODES)
   for (int iz = 0; iz < nz; ++iz)
     for (int iy = 0; iy < ny; ++iy)
       for (int ix = 0; ix < nx; ++ix)
@@ -308,7 +309,7 @@ int tslb_ref_init(tslb_ref *h, const double *phi, const double *u) {
   memcpy(h->u, u, 3 * N * sizeof(double));
   memset(h->pstar, 0, N * sizeof(double));          /* R9 */
   memset(h->A, 0, 6 * N * sizeof(double));          /* R9 */
-#pragma omp parallel for
+#pragma omp parallel for if (h->N >= OMP_MIN_NODES)
   for (int iz = 0; iz < h->nz; ++iz)
     for (int iy = 0; iy < h->ny; ++iy)
       for (int ix = 0; ix < h->nx; ++ix) {
@@ -326,7 +327,7 @@ int tslb_ref_init(tslb_ref *h, const double *phi, const double *u) {
  * from its own time-n macroscopic fields.  omega is local, from phi^n (R14, R15). */
 static void pass_collide(tslb_ref *h) {
   long N = h->N;
-#pragma omp parallel for
+#pragma omp parallel for if (h->N >= OMP_MIN_NODES)
   for (long x = 0; x < N; ++x) {
     double u[3] = {h->u[x], h->u[N + x], h->u[2 * N + x]};
     double a[3] = {h->a[x], h->a[N + x], h->a[2 * N + x]};
@@ -347,7 +348,7 @@ static void pass_collide(tslb_ref *h) {
 static void pass_stream(tslb_ref *h) {
   long N = h->N;
   const int *bc = h->p.bc;
-#pragma omp parallel for
+#pragma omp parallel for if (h->N >= OMP_MIN_NODES)
   for (int iz = 0; iz < h->nz; ++iz)
     for (int iy = 0; iy < h->ny; ++iy)
       for (int ix = 0; ix < h->nx; ++ix) {
@@ -369,7 +370,7 @@ static void pass_stream(tslb_ref *h) {
 static void pass_allen_cahn(tslb_ref *h) {
   long N = h->N;
   const int *bc = h->p.bc;
-#pragma omp parallel for
+#pragma omp parallel for if (h->N >= OMP_MIN_NODES)
   for (int iz = 0; iz < h->nz; ++iz)
     for (int iy = 0; iy < h->ny; ++iy)
       for (int ix = 0; ix < h->nx; ++ix) {
@@ -384,7 +385,7 @@ static void pass_allen_cahn(tslb_ref *h) {
       }
   /* the two fluxes as whole arrays: adv = phi u (velocity-like ghosts), shp = phi(1-phi) nrm
    * (normal-odd ghosts).  g is reused as scratch for adv, nrm is overwritten by shp. */
-#pragma omp parallel for
+#pragma omp parallel for if (h->N >= OMP_MIN_NODES)
   for (long x = 0; x < N; ++x) {
     double ph = h->phi[x];
     for (int al = 0; al < 3; ++al) {
@@ -392,7 +393,7 @@ static void pass_allen_cahn(tslb_ref *h) {
       h->nrm[al * N + x] = ph * (1.0 - ph) * h->nrm[al * N + x];
     }
   }
-#pragma omp parallel for
+#pragma omp parallel for if (h->N >= OMP_MIN_NODES)
   for (int iz = 0; iz < h->nz; ++iz)
     for (int iy = 0; iy < h->ny; ++iy)
       for (int ix = 0; ix < h->nx; ++ix) {
@@ -408,7 +409,7 @@ static void pass_allen_cahn(tslb_ref *h) {
  * R4), pre-regularisation (Eq. 13, computed literally with fbar_eq = feq - S/2). */
 static void pass_moments(tslb_ref *h) {
   long N = h->N;
-#pragma omp parallel for
+#pragma omp parallel for if (h->N >= OMP_MIN_NODES)
   for (int iz = 0; iz < h->nz; ++iz)
     for (int iy = 0; iy < h->ny; ++iy)
       for (int ix = 0; ix < h->nx; ++ix) {

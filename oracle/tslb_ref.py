@@ -23,8 +23,10 @@ def build_lib(force=False):
     if (not force and os.path.exists(_LIB)
             and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
         return _LIB
+    tmp = _LIB + f".{os.getpid()}.tmp"       # build aside, then rename: a process that has the
     subprocess.check_call(["gcc", "-O3", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-                           "-Wall", "-o", _LIB, _SRC, "-lm"])
+                           "-Wall", "-o", tmp, _SRC, "-lm"])       # old library mapped keeps it
+    os.replace(tmp, _LIB)
     return _LIB
 
 

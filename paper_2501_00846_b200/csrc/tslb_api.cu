@@ -51,7 +51,7 @@ bool params_ok(int nx, int ny, int nz, const tslb_params* p) {
 size_t elem_size(const tslb_params* p) { return p->precision == TSLB_F64 ? 8 : 4; }
 // bytes of one SoA plane, padded so that every plane starts 256-byte aligned
 size_t plane_bytes(long long N, size_t es) { return round_up(size_t(N) * es); }
-int scratch_planes(const tslb_params* p) { return (p->flags & TSLB_FLAG_NAIVE) ? 3 : 0; }
+int scratch_planes(const tslb_params*) { return 3; }   // Allen-Cahn flux Q (or naive scratch)
 
 template <typename T>
 tslb::DevParams<T> make_dev(int nx, int ny, int nz, const tslb_params& p, long long stride) {
@@ -79,7 +79,7 @@ struct tslb_handle {
   size_t es;
   cudaStream_t stream;
   char* buf[2];          // two state buffers of NFIELD planes
-  char* scratch;         // naive path only: 3 planes
+  char* scratch;         // 3 planes: flux Q of Eq. 20 (periodic path) / naive-path scratch
   int cur;
   bool inited;
   long long launches;
@@ -137,7 +137,8 @@ int init_impl(tslb_handle* h, const T* phi, const T* u, long long u_stride) {
   T* D = reinterpret_cast<T*>(h->buf[0]);
   h->cur = 0;
   unsigned blocks = unsigned((h->nodes + 255) / 256);
-  tslb::k_init<T><<<blocks, 256, 0, h->stream>>>(P, h->nodes, phi, u, u_stride, D);
+  tslb::k_init<T><<<blocks, 256, 0, h->stream>>>(P, h->nodes, phi, u, u_stride, D,
+                                                 reinterpret_cast<T*>(h->scratch));
   h->launches += 1;
   CUDA_TRY(cudaGetLastError());
   h->inited = true;
@@ -162,8 +163,8 @@ int step_impl(tslb_handle* h, int n, const tslb::Marker& mk) {
       mk.mark(TSLB_K_STREAM_COLLIDE);
       h->launches += 3;
     } else {
-      int rc = tslb::launch_step_tiled<T>(P, S, D, h->stream, &h->launches, mk,
-                                           h->prm.flags);
+      int rc = tslb::launch_step_tiled<T>(P, S, D, reinterpret_cast<T*>(h->scratch), h->stream,
+                                           &h->launches, mk, h->prm.flags);
       if (rc != 0) return fail(TSLB_ECUDA, "tiled launch: %s", cudaGetErrorString(cudaError_t(rc)));
     }
     h->cur ^= 1;

@@ -256,6 +256,35 @@ __device__ __forceinline__ Coef<T> coef_from13(const T (&m)[13]) {
                          m[F_AXZ], m[F_AYZ], m[F_AX], m[F_AY], m[F_AZ]);
 }
 
+// Total Allen-Cahn flux of Eq. 20 at one node (R13, R16):  Q = phi u + kappa_AC phi (1-phi) n,
+// n = grad(phi)/sqrt(|grad(phi)|^2 + eps^2).  The periodic path evaluates it where grad(phi^{n+1})
+// is already known (closing stage of the stream-collide kernel) and stores it for the next
+// step's interface update; layout: plane pair (Qx,Qy) at offset 0, plane Qz at offset 2N.
+template <typename T>
+__device__ __forceinline__ void flux_q(const DevParams<T>& P, T phi, T gx, T gy, T gz, T ux, T uy,
+                                       T uz, T (&q)[3]) {
+  const T s = P.kappa_ac * phi * (T(1) - phi) * rsqrt_t(gx * gx + gy * gy + gz * gz + T(1e-24));
+  q[0] = fma(phi, ux, s * gx);
+  q[1] = fma(phi, uy, s * gy);
+  q[2] = fma(phi, uz, s * gz);
+}
+__device__ __forceinline__ void store_q(double* Q, long long N, long long idx, const double (&q)[3]) {
+  reinterpret_cast<double2*>(Q)[idx] = make_double2(q[0], q[1]);
+  Q[2 * N + idx] = q[2];
+}
+__device__ __forceinline__ void store_q(float* Q, long long N, long long idx, const float (&q)[3]) {
+  reinterpret_cast<float2*>(Q)[idx] = make_float2(q[0], q[1]);
+  Q[2 * N + idx] = q[2];
+}
+__device__ __forceinline__ void load_q(const double* Q, long long N, long long idx, double (&q)[3]) {
+  const double2 v = __ldg(reinterpret_cast<const double2*>(Q) + idx);
+  q[0] = v.x; q[1] = v.y; q[2] = __ldg(Q + 2 * N + idx);
+}
+__device__ __forceinline__ void load_q(const float* Q, long long N, long long idx, float (&q)[3]) {
+  const float2 v = __ldg(reinterpret_cast<const float2*>(Q) + idx);
+  q[0] = v.x; q[1] = v.y; q[2] = __ldg(Q + 2 * N + idx);
+}
+
 // Ghost rule along one axis (R19): periodic wrap or even mirror about a wall half a cell outside
 // the first/last node.  Valid for -n <= i < 2n.  crossed = 1 if mirrored.
 __device__ __forceinline__ int ghost_index(int i, int n, int bc, int& crossed) {

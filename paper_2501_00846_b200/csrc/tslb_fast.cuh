@@ -187,7 +187,8 @@ template <int N> __device__ __forceinline__ void cp_async_wait() {
 // NSTAGE > 0 : cp.async staging NSTAGE planes ahead (PREFETCH is then ignored)
 template <typename T, int TX, int TY, int MINB, bool PREFETCH, int ABL = 0, int NSTAGE = 0>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
-k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D, int zchunk) {
+k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D,
+                      T* __restrict__ Qout, int zchunk) {
   using M = TileMap<TX, TY, 1>;
   using SM = K2FastSmem<T, M::CELLS>;
   using STG = StageBuf<T, M::CELLS>;
@@ -411,6 +412,11 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         if (ABL & 2) { out.p = m.p + lap; out.ux = m.mx + gx_; out.uy = m.my + gy_; out.uz = m.mz + gz_; out.axx = m.xx; out.ayy = m.yy; out.azz = m.zz; out.axy = m.xy; out.axz = m.xz; out.ayz = m.yz; out.ax = uPrev[0]; out.ay = uPrev[1]; out.az = uPrev[2]; }
         else out = close_node(P, m, ph_0, gx_, gy_, gz_, lap, uPrev[0], uPrev[1], uPrev[2]);
         if (!(ABL & 4) || out.p == T(123.456)) store_out(D, P.N, gx + P.nx * gy + plane * k, out);
+        if (Qout != nullptr && !(ABL & 4)) {        // flux of Eq. 20 for the next step (K1 flux form)
+          T q[3];
+          flux_q(P, ph_0, gx_, gy_, gz_, out.ux, out.uy, out.uz, q);
+          store_q(Qout, P.N, gx + P.nx * gy + plane * k, q);
+        }
       }
       // slot A is free now: it becomes the accumulator of destination plane j+1
 #pragma unroll

@@ -1,0 +1,132 @@
+// tslb_flux.cuh -- interface tracking (Eq. 20) in FLUX FORM for all-periodic boxes.
+//
+//   phi^{n+1} = phi - div Q + D lap(phi),   Q = phi u + kappa_AC phi (1-phi) n   (R13, R16)
+//
+// The normal n needs grad(phi^n), which the stream-collide kernel of the PREVIOUS step already
+// computed for the forces (phi^n is that step's phi^{n+1}).  So that kernel (and tslb_init for
+// the first step) stores Q, and this kernel is left with one radius-1 stencil pass: no ring of
+// depth 2, no normalisation, no second barrier.  Per node and plane:
+//   * z-combinations of the own column (Eq. 18/19 are separable):
+//       X = Qx(k-1) + 4 Qx(k) + Qx(k+1),  Y likewise,  Z = Qz(k+1) - Qz(k-1),
+//       pz = phi(k-1) + 4 phi(k) + phi(k+1);
+//   * with A = c1 Z + c2 pz, Bx = c1 X, By = c1 Y  (c1 = -3/216, c2 = 6 D/216) the node SCATTERS
+//     w(dx) w(dy) (A - dx Bx - dy By) to its 8 in-plane neighbours (integer weights (1,4,1));
+//   * the receiver adds its 8 arrivals, its own 16 A and (1 - 6 D) phi(k).
+// Walls use k_allen_cahn_tiled (ghost rules differ for the two parts of Q, R19).
+#pragma once
+#include "tslb_fast.cuh"
+#include "tslb_tiled.cuh"
+
+namespace tslb {
+
+template <typename T, int CELLS>
+struct FluxBuf { typename Pair2<T>::type dv[4][CELLS]; };   // 8 direction scalars, paired
+// cp.async staging slot of one plane: (Qx,Qy), Qz, phi of the thread's own node
+template <typename T, int CELLS>
+struct FluxStage { typename Pair2<T>::type qxy[CELLS]; T qz[CELLS]; T ph[CELLS]; };
+__device__ __forceinline__ void cp_async_pair(double2* dst, const double2* src) { cp_async16(dst, src); }
+__device__ __forceinline__ void cp_async_pair(float2* dst, const float2* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(dst)), "l"(src));
+}
+
+// NSTAGE planes are kept in flight per thread through cp.async (the kernel moves 40 / 20 bytes
+// per update: without a deep memory pipeline it is bound by latency, not bandwidth).
+template <typename T, int TX, int TY, int MINB, int NSTAGE>
+__global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
+k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ Q,
+                  T* __restrict__ phin, int zchunk) {
+  using M = TileMap<TX, TY, 1>;
+  using P2 = typename Pair2<T>::type;
+  extern __shared__ __align__(16) unsigned char flux_smem_raw[];
+  FluxBuf<T, M::CELLS>* sm = reinterpret_cast<FluxBuf<T, M::CELLS>*>(flux_smem_raw);
+  FluxStage<T, M::CELLS>* stg = reinterpret_cast<FluxStage<T, M::CELLS>*>(
+      flux_smem_raw + 2 * sizeof(FluxBuf<T, M::CELLS>));
+
+  const int tid = threadIdx.x;
+  int lx, ly;
+  const bool mapped = M::coords(tid, lx, ly);
+  const int gx = blockIdx.x * TX + lx, gy = blockIdx.y * TY + ly;
+  const int z0 = blockIdx.z * zchunk;
+  const int z1 = min(P.nz, z0 + zchunk);
+  const int c = M::cell(lx, ly);
+  const bool in_ring = mapped && gx >= -1 && gx <= P.nx && gy >= -1 && gy <= P.ny;
+  const bool is_out = tid < M::NMAIN && gx < P.nx && gy < P.ny;
+  const int sx = gx < 0 ? gx + P.nx : (gx >= P.nx ? gx - P.nx : gx);
+  const int sy = gy < 0 ? gy + P.ny : (gy >= P.ny ? gy - P.ny : gy);
+  const int plane = P.nx * P.ny;
+  const int col = in_ring ? sx + P.nx * sy : 0;
+  const T* phi = S + F_PHI * P.N;
+  const T c1 = T(-3.0 / 216.0), c2 = P.mob * T(6.0 / 216.0), c0 = T(1) - T(6) * P.mob;
+
+  auto load = [&](int z, T (&q)[3], T& f) {
+    const int jz = z < 0 ? z + P.nz : (z >= P.nz ? z - P.nz : z);
+    const int s = col + plane * jz;
+    load_q(Q, P.N, s, q);
+    f = __ldg(phi + s);
+  };
+
+  auto stage_issue = [&](int z, int slot) {
+    if (in_ring && z <= z1) {
+      const int jz = z < 0 ? z + P.nz : (z >= P.nz ? z - P.nz : z);
+      const int s = col + plane * jz;
+      cp_async_pair(&stg[slot].qxy[c], reinterpret_cast<const P2*>(Q) + s);
+      cp_async_small(&stg[slot].qz[c], Q + 2 * P.N + s);
+      cp_async_small(&stg[slot].ph[c], phi + s);
+    }
+    cp_async_commit();
+  };
+
+  // own column at planes k-1 (a), k (b), k+1 (c)
+  T qa[3] = {}, qb[3] = {}, qc[3] = {}, fa = 0, fb = 0, fc = 0;
+  if (in_ring) {
+    load(z0 - 1, qb, fb);
+    load(z0, qc, fc);
+  }
+#pragma unroll
+  for (int d = 0; d < NSTAGE; ++d) stage_issue(z0 + 1 + d, d);
+
+  int slot = 0;
+  for (int k = z0; k < z1; ++k) {
+    FluxBuf<T, M::CELLS>& w = sm[(k - z0) & 1];
+    T own = 0;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { qa[i] = qb[i]; qb[i] = qc[i]; }
+    fa = fb; fb = fc;
+    cp_async_wait<NSTAGE - 1>();                 // plane k+1 of the own column has landed
+    if (in_ring) {
+      const P2 v = stg[slot].qxy[c];
+      qc[0] = v.x; qc[1] = v.y; qc[2] = stg[slot].qz[c]; fc = stg[slot].ph[c];
+    }
+    stage_issue(k + 1 + NSTAGE, slot);
+    slot = (slot + 1 == NSTAGE) ? 0 : slot + 1;
+    if (in_ring) {
+      const T X = fma(T(4), qb[0], qa[0] + qc[0]);
+      const T Y = fma(T(4), qb[1], qa[1] + qc[1]);
+      const T Z = qc[2] - qa[2];
+      const T pz = fma(T(4), fb, fa + fc);
+      const T A = fma(c1, Z, c2 * pz), Bx = c1 * X, By = c1 * Y;
+      own = T(16) * A;
+      const T apx = A + Bx, amx = A - Bx;
+      // direction d = (dx,dy): slots (-1,-1) (0,-1) | (1,-1) (-1,0) | (1,0) (-1,1) | (0,1) (1,1)
+      P2 v;
+      v.x = apx + By;            v.y = T(4) * (A + By);   w.dv[0][c] = v;
+      v.x = amx + By;            v.y = T(4) * apx;        w.dv[1][c] = v;
+      v.x = T(4) * amx;          v.y = apx - By;          w.dv[2][c] = v;
+      v.x = T(4) * (A - By);     v.y = amx - By;          w.dv[3][c] = v;
+    }
+    __syncthreads();
+    if (is_out) {
+      // the value sent in direction d arrives from the source at -d
+      T s = own;
+      s += (w.dv[0][c + M::W + 1].x + w.dv[3][c - M::W - 1].y)      // (-1,-1) , (1,1)
+         + (w.dv[1][c + M::W - 1].x + w.dv[2][c - M::W + 1].y);     // (1,-1)  , (-1,1)
+      s += (w.dv[0][c + M::W].y + w.dv[3][c - M::W].x)              // (0,-1)  , (0,1)
+         + (w.dv[1][c + 1].y + w.dv[2][c - 1].x);                   // (-1,0)  , (1,0)
+      phin[gx + P.nx * gy + plane * k] = fma(c0, fb, s);
+    }
+  }
+  cp_async_wait<0>();
+}
+
+}  // namespace tslb

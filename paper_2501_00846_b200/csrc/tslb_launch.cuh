@@ -1,6 +1,7 @@
 // tslb_launch.cuh -- launch of one time step: kernel selection, grid sizing, attributes.
 #pragma once
 #include "tslb_fast.cuh"
+#include "tslb_flux.cuh"
 #include "tslb_stag.cuh"
 #include "tslb_tiled.cuh"
 
@@ -18,7 +19,7 @@ inline cudaError_t prepare(K kernel, size_t smem) {
 }
 
 template <typename T, int TY, int MINB, bool PREFETCH, int ABL = 0, int NSTAGE = 0>
-cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream) {
+cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream) {
   constexpr int TX = 32;
   using M = TileMap<TX, TY, 1>;
   auto kernel = k_stream_collide_fast<T, TX, TY, MINB, PREFETCH, ABL, NSTAGE>;
@@ -30,12 +31,12 @@ cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, cudaStream_t st
     ready = true;
   }
   const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
-  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, ZCHUNK);
+  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, Q, ZCHUNK);
   return cudaGetLastError();
 }
 
 template <typename T, int TY, int MINB>
-cudaError_t launch_stag(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream) {
+cudaError_t launch_stag(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream) {
   constexpr int TX = 32;
   using M = TileMap<TX, TY, 1>;
   auto kernel = k_stream_collide_stag<T, TX, TY, MINB>;
@@ -47,7 +48,7 @@ cudaError_t launch_stag(const DevParams<T>& P, const T* S, T* D, cudaStream_t st
     ready = true;
   }
   const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
-  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, ZCHUNK);
+  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, Q, ZCHUNK);
   return cudaGetLastError();
 }
 
@@ -65,6 +66,23 @@ cudaError_t launch_generic(const DevParams<T>& P, const T* S, T* D, cudaStream_t
   }
   const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
   kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, ZCHUNK);
+  return cudaGetLastError();
+}
+
+template <typename T, int TY, int MINB, int NSTAGE>
+cudaError_t launch_k1_flux(const DevParams<T>& P, const T* S, const T* Q, T* D, cudaStream_t stream) {
+  constexpr int TX = 32;
+  using M = TileMap<TX, TY, 1>;
+  auto kernel = k_allen_cahn_flux<T, TX, TY, MINB, NSTAGE>;
+  const size_t smem = 2 * sizeof(FluxBuf<T, M::CELLS>) + NSTAGE * sizeof(FluxStage<T, M::CELLS>);
+  static bool ready = false;
+  if (!ready) {
+    cudaError_t e = prepare(kernel, smem);
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
+  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, Q, D + F_PHI * P.N, ZCHUNK);
   return cudaGetLastError();
 }
 
@@ -93,15 +111,23 @@ cudaError_t launch_k1(const DevParams<T>& P, const T* S, T* D, cudaStream_t stre
 
 // variant = (flags >> 8) & 0xff : tuning selector, 0 = production choice.
 template <typename T>
-int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream,
+int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
                       long long* launches, const Marker& mk, int flags) {
   const bool walls = P.bcx || P.bcy || P.bcz;
   const bool generic = walls || (flags & 2);
   const int variant = (flags >> 8) & 0xff;
   cudaError_t e;
-  switch ((flags >> 16) & 0xf) {     // bits 16-19: tuning variant of the Allen-Cahn kernel
+  const int k1v = (flags >> 16) & 0xf;   // bits 16-19: tuning variant of the Allen-Cahn kernel
+  const bool flux_form = !(P.bcx || P.bcy || P.bcz) && !(flags & 2) && (k1v == 0 || k1v >= 5);
+  switch (flux_form ? 100 + k1v : k1v) {
+    case 100: e = launch_k1_flux<T, 8, 2, 3>(P, S, Q, D, stream); break;   // production, periodic
+    case 105: e = launch_k1_flux<T, 8, 3, 2>(P, S, Q, D, stream); break;
+    case 106: e = launch_k1_flux<T, 8, 3, 4>(P, S, Q, D, stream); break;
+    case 107: e = launch_k1_flux<T, 16, 2, 3>(P, S, Q, D, stream); break;
+    case 108: e = launch_k1_flux<T, 8, 2, 1>(P, S, Q, D, stream); break;
+    case 109: e = launch_k1_flux<T, 8, 4, 4>(P, S, Q, D, stream); break;
     default:
-    case 0: e = launch_k1<T, 8, 2>(P, S, D, stream); break;
+    case 0: case 4: e = launch_k1<T, 8, 2>(P, S, D, stream); break;
     case 1: e = launch_k1<T, 16, 1>(P, S, D, stream); break;
     case 2: e = launch_k1<T, 8, 1>(P, S, D, stream); break;
     case 3: e = launch_k1<T, 4, 3>(P, S, D, stream); break;
@@ -114,33 +140,33 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, cudaStream_t stre
     switch (variant) {
       default:   // production choice: fp64 one block/SM, fp32 two blocks/SM
       case 0:
-        e = sizeof(T) == 8 ? launch_fast<T, 8, 1, false, 0, 1>(P, S, D, stream)
-                           : launch_fast<T, 8, 2, false, 0, 1>(P, S, D, stream);
+        e = sizeof(T) == 8 ? launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream)
+                           : launch_fast<T, 8, 2, false, 0, 1>(P, S, D, Q, stream);
         break;
-      case 6: e = launch_fast<T, 8, 1, false>(P, S, D, stream); break;
-      case 7: e = launch_fast<T, 4, 2, false>(P, S, D, stream); break;
-      case 21: e = launch_fast<T, 8, 1, false, 4, 1>(P, S, D, stream); break;    // timing ablations
-      case 22: e = launch_fast<T, 8, 1, false, 8, 1>(P, S, D, stream); break;
-      case 23: e = launch_fast<T, 8, 1, false, 12, 1>(P, S, D, stream); break;
-      case 24: e = launch_fast<T, 8, 1, false, 16, 1>(P, S, D, stream); break;
-      case 25: e = launch_fast<T, 8, 1, false, 1 + 2 + 32, 1>(P, S, D, stream); break;
-      case 26: e = launch_fast<T, 8, 1, false, 1 + 2 + 16 + 32, 1>(P, S, D, stream); break;
-      case 27: e = launch_fast<T, 8, 1, false, 1, 1>(P, S, D, stream); break;
-      case 28: e = launch_fast<T, 8, 1, false, 2, 1>(P, S, D, stream); break;
-      case 29: e = launch_fast<T, 8, 1, false, 32, 1>(P, S, D, stream); break;
-      case 30: e = launch_fast<T, 8, 1, false, 0, 1>(P, S, D, stream); break;   // cp.async staging
-      case 31: e = launch_fast<T, 8, 1, false, 0, 2>(P, S, D, stream); break;
-      case 32: e = launch_fast<T, 8, 2, false, 0, 1>(P, S, D, stream); break;
-      case 10: e = launch_stag<T, 8, 1>(P, S, D, stream); break;
-      case 11: e = launch_stag<T, 8, 2>(P, S, D, stream); break;
-      case 12: e = launch_stag<T, 4, 2>(P, S, D, stream); break;
-      case 8: e = launch_fast<T, 4, 2, true>(P, S, D, stream); break;
-      case 9: e = launch_fast<T, 4, 3, false>(P, S, D, stream); break;
-      case 1: e = launch_fast<T, 8, 1, true>(P, S, D, stream); break;
-      case 2: e = launch_fast<T, 8, 2, false>(P, S, D, stream); break;
-      case 3: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, false>(P, S, D, stream); break;
-      case 4: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, true>(P, S, D, stream); break;
-      case 5: e = launch_fast<T, 8, 2, true>(P, S, D, stream); break;
+      case 6: e = launch_fast<T, 8, 1, false>(P, S, D, Q, stream); break;
+      case 7: e = launch_fast<T, 4, 2, false>(P, S, D, Q, stream); break;
+      case 21: e = launch_fast<T, 8, 1, false, 4, 1>(P, S, D, Q, stream); break;    // timing ablations
+      case 22: e = launch_fast<T, 8, 1, false, 8, 1>(P, S, D, Q, stream); break;
+      case 23: e = launch_fast<T, 8, 1, false, 12, 1>(P, S, D, Q, stream); break;
+      case 24: e = launch_fast<T, 8, 1, false, 16, 1>(P, S, D, Q, stream); break;
+      case 25: e = launch_fast<T, 8, 1, false, 1 + 2 + 32, 1>(P, S, D, Q, stream); break;
+      case 26: e = launch_fast<T, 8, 1, false, 1 + 2 + 16 + 32, 1>(P, S, D, Q, stream); break;
+      case 27: e = launch_fast<T, 8, 1, false, 1, 1>(P, S, D, Q, stream); break;
+      case 28: e = launch_fast<T, 8, 1, false, 2, 1>(P, S, D, Q, stream); break;
+      case 29: e = launch_fast<T, 8, 1, false, 32, 1>(P, S, D, Q, stream); break;
+      case 30: e = launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream); break;   // cp.async staging
+      case 31: e = launch_fast<T, 8, 1, false, 0, 2>(P, S, D, Q, stream); break;
+      case 32: e = launch_fast<T, 8, 2, false, 0, 1>(P, S, D, Q, stream); break;
+      case 10: e = launch_stag<T, 8, 1>(P, S, D, Q, stream); break;
+      case 11: e = launch_stag<T, 8, 2>(P, S, D, Q, stream); break;
+      case 12: e = launch_stag<T, 4, 2>(P, S, D, Q, stream); break;
+      case 8: e = launch_fast<T, 4, 2, true>(P, S, D, Q, stream); break;
+      case 9: e = launch_fast<T, 4, 3, false>(P, S, D, Q, stream); break;
+      case 1: e = launch_fast<T, 8, 1, true>(P, S, D, Q, stream); break;
+      case 2: e = launch_fast<T, 8, 2, false>(P, S, D, Q, stream); break;
+      case 3: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, false>(P, S, D, Q, stream); break;
+      case 4: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, true>(P, S, D, Q, stream); break;
+      case 5: e = launch_fast<T, 8, 2, true>(P, S, D, Q, stream); break;
     }
   }
   mk.mark(2);

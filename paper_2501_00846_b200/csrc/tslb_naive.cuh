@@ -176,7 +176,7 @@ template <typename T>
 __global__ void __launch_bounds__(256) k_init(DevParams<T> P, long long nodes,
                                               const T* __restrict__ phi0,
                                               const T* __restrict__ u0, long long us,
-                                              T* __restrict__ D) {
+                                              T* __restrict__ D, T* __restrict__ Q) {
   long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (idx >= nodes) return;
   int ix, iy, iz;
@@ -194,6 +194,9 @@ __global__ void __launch_bounds__(256) k_init(DevParams<T> P, long long nodes,
   o.az = fma(db, P.gz, mu_phi * gz) * mx.inv_rho;
   store_node(D, P.N, idx, o);
   D[F_PHI * P.N + idx] = ph;
+  T q[3];                                    // flux of Eq. 20 for the first interface update
+  flux_q(P, ph, gx, gy, gz, o.ux, o.uy, o.uz, q);
+  store_q(Q, P.N, idx, q);
 }
 
 // ---- tslb_get: rho, p = p* rho cs^2, u, phi

@@ -21,7 +21,8 @@ namespace tslb {
 
 template <typename T, int TX, int TY, int MINB>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
-k_stream_collide_stag(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D, int zchunk) {
+k_stream_collide_stag(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D,
+                      T* __restrict__ Qout, int zchunk) {
   using M = TileMap<TX, TY, 1>;
   using SM = K2FastSmem<T, M::CELLS>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -154,6 +155,11 @@ k_stream_collide_stag(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
       const T lap = fma(T(6.0 / 216.0), sw, T(-6) * phk);
       const NodeOut<T> out = close_node(P, m, phk, gx_, gy_, gz_, lap, uk[0], uk[1], uk[2]);
       store_out(D, P.N, gx + P.nx * gy + plane * k, out);
+      if (Qout != nullptr) {
+        T q[3];
+        flux_q(P, phk, gx_, gy_, gz_, out.ux, out.uy, out.uz, q);
+        store_q(Qout, P.N, gx + P.nx * gy + plane * k, q);
+      }
     }
 #pragma unroll
     for (int i = 0; i < 6; ++i) aA[i] = up[i];

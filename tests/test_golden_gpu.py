@@ -14,7 +14,7 @@ HERE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 CASES = {
     "droplet32": lambda: I.static_droplet(32, 8.0, seed=1),
     "collision64": lambda: I.head_on_collision(n=64, radius=6.0, half_sep=10.0),
-    "bubble32x32x64": lambda: I.rising_bubble(nx=32, ny=32, nz=64, radius=4.0, height=10.0),
+    "bubble48x48x96": lambda: I.rising_bubble(nx=48, ny=48, nz=96, radius=8.0, height=20.0),
     "laplace128_R12": lambda: I.static_droplet(128, 12.0, seed=12),
 }
 
@@ -59,8 +59,13 @@ def test_against_golden(case, precision):
         print(f"[{case} {precision}] step {cp}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items())
               + f" | sum(phi) rel diff {sum_phi / gold[f'diag_{cp}'][0] - 1:.1e}"
               + f" sum(p*) {sum_ps:.1e} (oracle {gold[f'diag_{cp}'][1]:.1e})")
-        worst[cp] = {k: errs[k] for k in fields}
+        # the bar: BASELINE.json's tolerance, widened to 10 x the trajectory's own sensitivity to
+        # a 1e-15 input perturbation where the oracle recorded one
+        sens = dict(zip(("rho", "p", "u", "phi"), gold[f"sens_{cp}"])) if f"sens_{cp}" in gold else {}
+        worst[cp] = {k: (errs[k], max(tol, 10.0 * float(sens.get(k, 0.0)))) for k in fields}
+        if sens:
+            print(f"    oracle sensitivity: " + " ".join(f"{k}={v:.1e}" for k, v in sens.items()))
         assert bool(torch.isfinite(g["u"]).all())
     s.close()
-    bad = {cp: e for cp, e in worst.items() if any(not (v <= tol) for v in e.values())}
+    bad = {cp: e for cp, e in worst.items() if any(not (v <= bar) for v, bar in e.values())}
     assert not bad, bad
