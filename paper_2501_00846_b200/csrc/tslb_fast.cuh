@@ -22,8 +22,8 @@ __host__ __device__ constexpr int dir_slot(int cx, int cy) {
 }
 
 // Exchange buffers, double buffered over the marching index so that one __syncthreads per plane
-// is enough.  fp64: (E,O) as one 128-bit word + Qq as a 64-bit word per direction and cell;
-// fp32: (E,O,Qq,-) as one 128-bit word.
+// is enough.  Per direction and cell: (E,O) as one pair word (128 bit in fp64, 64 bit in fp32)
+// and Qq as a scalar; every access is contiguous across the warp (no bank conflicts).
 template <typename T, int CELLS> struct ExBuf;
 template <int CELLS> struct ExBuf<double, CELLS> {
   double2 eo[8][CELLS];
@@ -47,19 +47,21 @@ template <int CELLS> struct ExBuf<double, CELLS> {
   }
 };
 template <int CELLS> struct ExBuf<float, CELLS> {
-  float4 eoq[8][CELLS];
+  float2 eo[8][CELLS];
+  float q[8][CELLS];
   float2 pd[CELLS];
   __device__ __forceinline__ void put(int slot, int c, float E, float O, float Q) {
-    eoq[slot][c] = make_float4(E, O, Q, 0.f);
+    eo[slot][c] = make_float2(E, O);
+    q[slot][c] = Q;
   }
   __device__ __forceinline__ void get(int slot, int c, float& E, float& O, float& Q) const {
-    const float4 v = eoq[slot][c];
-    E = v.x; O = v.y; Q = v.z;
+    const float2 v = eo[slot][c];
+    E = v.x; O = v.y; Q = q[slot][c];
   }
   __device__ __forceinline__ void get_eo(int slot, int c, float& E, float& O) const {
-    const float4 v = eoq[slot][c]; E = v.x; O = v.y;
+    const float2 v = eo[slot][c]; E = v.x; O = v.y;
   }
-  __device__ __forceinline__ void get_q(int slot, int c, float& Q) const { Q = eoq[slot][c].z; }
+  __device__ __forceinline__ void get_q(int slot, int c, float& Q) const { Q = q[slot][c]; }
   __device__ __forceinline__ void put_pd(int c, float a, float b) { pd[c] = make_float2(a, b); }
   __device__ __forceinline__ void get_pd(int c, float& a, float& b) const {
     const float2 v = pd[c]; a = v.x; b = v.y;

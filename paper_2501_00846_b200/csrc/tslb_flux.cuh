@@ -20,7 +20,7 @@
 namespace tslb {
 
 template <typename T, int CELLS>
-struct FluxBuf { typename Pair2<T>::type dv[4][CELLS]; };   // 8 direction scalars, paired
+struct FluxBuf { T dv[8][CELLS]; };   // 8 direction scalars (separate arrays: conflict-free reads)
 // cp.async staging slot of one plane: (Qx,Qy), Qz, phi of the thread's own node
 template <typename T, int CELLS>
 struct FluxStage { typename Pair2<T>::type qxy[CELLS]; T qz[CELLS]; T ph[CELLS]; };
@@ -108,21 +108,20 @@ k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__
       const T A = fma(c1, Z, c2 * pz), Bx = c1 * X, By = c1 * Y;
       own = T(16) * A;
       const T apx = A + Bx, amx = A - Bx;
-      // direction d = (dx,dy): slots (-1,-1) (0,-1) | (1,-1) (-1,0) | (1,0) (-1,1) | (0,1) (1,1)
-      P2 v;
-      v.x = apx + By;            v.y = T(4) * (A + By);   w.dv[0][c] = v;
-      v.x = amx + By;            v.y = T(4) * apx;        w.dv[1][c] = v;
-      v.x = T(4) * amx;          v.y = apx - By;          w.dv[2][c] = v;
-      v.x = T(4) * (A - By);     v.y = amx - By;          w.dv[3][c] = v;
+      // direction d = (dx,dy): slots 0..7 = (-1,-1) (0,-1) (1,-1) (-1,0) (1,0) (-1,1) (0,1) (1,1)
+      w.dv[0][c] = apx + By;            w.dv[1][c] = T(4) * (A + By);
+      w.dv[2][c] = amx + By;            w.dv[3][c] = T(4) * apx;
+      w.dv[4][c] = T(4) * amx;          w.dv[5][c] = apx - By;
+      w.dv[6][c] = T(4) * (A - By);     w.dv[7][c] = amx - By;
     }
     __syncthreads();
     if (is_out) {
       // the value sent in direction d arrives from the source at -d
       T s = own;
-      s += (w.dv[0][c + M::W + 1].x + w.dv[3][c - M::W - 1].y)      // (-1,-1) , (1,1)
-         + (w.dv[1][c + M::W - 1].x + w.dv[2][c - M::W + 1].y);     // (1,-1)  , (-1,1)
-      s += (w.dv[0][c + M::W].y + w.dv[3][c - M::W].x)              // (0,-1)  , (0,1)
-         + (w.dv[1][c + 1].y + w.dv[2][c - 1].x);                   // (-1,0)  , (1,0)
+      s += (w.dv[0][c + M::W + 1] + w.dv[7][c - M::W - 1])          // (-1,-1) , (1,1)
+         + (w.dv[2][c + M::W - 1] + w.dv[5][c - M::W + 1]);         // (1,-1)  , (-1,1)
+      s += (w.dv[1][c + M::W] + w.dv[6][c - M::W])                  // (0,-1)  , (0,1)
+         + (w.dv[3][c + 1] + w.dv[4][c - 1]);                       // (-1,0)  , (1,0)
       phin[gx + P.nx * gy + plane * k] = fma(c0, fb, s);
     }
   }
