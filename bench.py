@@ -24,6 +24,10 @@ sys.path.insert(0, ROOT)
 
 METRIC = "GLUPS per B200 (fp32/fp64) and % of HBM roofline on 256^3 droplet domain"
 STATE_SCALARS = 14                      # p*, u(3), Ahat(6), a(3), phi  -> 28 s bytes per update
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel on the 256^3
+# workload, from the ncu --set full captures summarised in profiles/r1_final_kernels_{f64,f32}.txt
+NCU_TRAFFIC = {("f64", "stream_collide"): 2.015428e9 + 2.104042e9,
+               ("f32", "stream_collide"): 0.969530e9 + 1.030411e9}
 
 
 def parse():
@@ -285,13 +289,17 @@ def main():
         # whole update, 28 s per node, charged to the dominant kernel's own duration only when
         # the step is a single kernel; for a split step each kernel is charged its own planes.
         dom = max(r["kernel_ms"], key=r["kernel_ms"].get)
-        planes = {"stream_collide": 27 if len(r["kernel_ms"]) > 1 else 28, "allen_cahn": 5,
-                  "normal": 4}[dom]
+        # scalars per update the dominant kernel must move: the periodic
+        # stream-collide kernel reads 13 moments + phi^{n+1} and writes 13 moments + the flux Q (3);
+        # the wall-capable / naive one writes no Q.
+        periodic_fast = not (args.naive or args.generic) and not any(cfg["params"]["bc"])
+        planes = {"stream_collide": 30 if periodic_fast else 27, "allen_cahn": 5, "normal": 4}[dom]
         k_ms = r["kernel_ms"][dom] / args.steps
         ach = planes * es * n / (k_ms * 1e-3) / 1e9
         step_ach = 2 * STATE_SCALARS * es * n / (r["ms"] / args.steps * 1e-3) / 1e9
         r["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak,
-                         "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                         "unit": "GB/s", "frac": ach / peak,
+                         "traffic": NCU_TRAFFIC.get((prec, dom)) if (periodic_fast and n == 256 ** 3) else None,
                          "peak_kind": peak_kind, "kernel_ms": k_ms,
                          "kernel_share_of_step": r["kernel_ms"][dom] / r["ms"],
                          "algorithmic_bytes_per_update": planes * es,
