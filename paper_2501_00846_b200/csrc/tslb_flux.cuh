@@ -83,23 +83,35 @@ k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__
     load(z0 - 1, qb, fb);
     load(z0, qc, fc);
   }
+  if (NSTAGE > 0) {
 #pragma unroll
-  for (int d = 0; d < NSTAGE; ++d) stage_issue(z0 + 1 + d, d);
+    for (int d = 0; d < NSTAGE; ++d) stage_issue(z0 + 1 + d, d);
+  }
+  // NSTAGE == 0: planes k+1 and k+2 wait in two register sets that alternate (loop unrolled by 2)
+  T r0q[3] = {}, r1q[3] = {}, r0f = 0, r1f = 0;
+  if (NSTAGE == 0 && in_ring) {
+    load(z0 + 1, r0q, r0f);
+    load(z0 + 2, r1q, r1f);
+  }
 
   int slot = 0;
-  for (int k = z0; k < z1; ++k) {
-    FluxBuf<T, M::CELLS>& w = sm[(k - z0) & 1];
+  auto step = [&](const int k, FluxBuf<T, M::CELLS>& w, T (&rq)[3], T& rf) {
     T own = 0;
 #pragma unroll
     for (int i = 0; i < 3; ++i) { qa[i] = qb[i]; qb[i] = qc[i]; }
     fa = fb; fb = fc;
-    cp_async_wait<NSTAGE - 1>();                 // plane k+1 of the own column has landed
-    if (in_ring) {
-      const P2 v = stg[slot].qxy[c];
-      qc[0] = v.x; qc[1] = v.y; qc[2] = stg[slot].qz[c]; fc = stg[slot].ph[c];
+    if (NSTAGE > 0) {
+      cp_async_wait<(NSTAGE > 0 ? NSTAGE - 1 : 0)>();   // plane k+1 of the own column has landed
+      if (in_ring) {
+        const P2 v = stg[slot].qxy[c];
+        qc[0] = v.x; qc[1] = v.y; qc[2] = stg[slot].qz[c]; fc = stg[slot].ph[c];
+      }
+      stage_issue(k + 1 + NSTAGE, slot);
+      slot = (slot + 1 == NSTAGE) ? 0 : slot + 1;
+    } else if (in_ring) {
+      qc[0] = rq[0]; qc[1] = rq[1]; qc[2] = rq[2]; fc = rf;
+      if (k + 3 <= z1) load(k + 3, rq, rf);
     }
-    stage_issue(k + 1 + NSTAGE, slot);
-    slot = (slot + 1 == NSTAGE) ? 0 : slot + 1;
     if (in_ring) {
       const T X = fma(T(4), qb[0], qa[0] + qc[0]);
       const T Y = fma(T(4), qb[1], qa[1] + qc[1]);
@@ -124,8 +136,12 @@ k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__
          + (w.dv[3][c + 1] + w.dv[4][c - 1]);                       // (-1,0)  , (1,0)
       phin[gx + P.nx * gy + plane * k] = fma(c0, fb, s);
     }
+  };
+  for (int k = z0; k < z1; k += 2) {
+    step(k, sm[0], r0q, r0f);
+    if (k + 1 < z1) step(k + 1, sm[1], r1q, r1f);
   }
-  cp_async_wait<0>();
+  if (NSTAGE > 0) cp_async_wait<0>();
 }
 
 }  // namespace tslb

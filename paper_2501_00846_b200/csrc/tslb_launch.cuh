@@ -18,9 +18,8 @@ inline cudaError_t prepare(K kernel, size_t smem) {
                               cudaSharedmemCarveoutMaxShared);
 }
 
-template <typename T, int TY, int MINB, bool PREFETCH, int ABL = 0, int NSTAGE = 0>
+template <typename T, int TY, int MINB, bool PREFETCH, int ABL = 0, int NSTAGE = 0, int TX = 32>
 cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream) {
-  constexpr int TX = 32;
   using M = TileMap<TX, TY, 1>;
   auto kernel = k_stream_collide_fast<T, TX, TY, MINB, PREFETCH, ABL, NSTAGE>;
   const size_t smem = sizeof(K2FastSmem<T, M::CELLS>) + NSTAGE * sizeof(StageBuf<T, M::CELLS>);
@@ -124,7 +123,9 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
     case 105: e = launch_k1_flux<T, 8, 3, 2>(P, S, Q, D, stream); break;
     case 106: e = launch_k1_flux<T, 8, 3, 4>(P, S, Q, D, stream); break;
     case 107: e = launch_k1_flux<T, 16, 2, 3>(P, S, Q, D, stream); break;
-    case 108: e = launch_k1_flux<T, 8, 2, 1>(P, S, Q, D, stream); break;
+    case 108: e = launch_k1_flux<T, 8, 2, 0>(P, S, Q, D, stream); break;   // register prefetch x2
+    case 110: e = launch_k1_flux<T, 8, 3, 0>(P, S, Q, D, stream); break;
+    case 111: e = launch_k1_flux<T, 16, 2, 0>(P, S, Q, D, stream); break;
     case 109: e = launch_k1_flux<T, 8, 4, 4>(P, S, Q, D, stream); break;
     default:
     case 0: case 4: e = launch_k1<T, 8, 2>(P, S, D, stream); break;
@@ -157,6 +158,13 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
       case 30: e = launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream); break;   // cp.async staging
       case 31: e = launch_fast<T, 8, 1, false, 0, 2>(P, S, D, Q, stream); break;
       case 32: e = launch_fast<T, 8, 2, false, 0, 1>(P, S, D, Q, stream); break;
+      case 36: e = launch_fast<T, 4, 2, false, 0, 1>(P, S, D, Q, stream); break;
+      case 37: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, false, 0, 1>(P, S, D, Q, stream); break;
+      case 38: e = launch_fast<T, 4, 3, false, 0, 1>(P, S, D, Q, stream); break;
+      case 39: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, false, 0, 2>(P, S, D, Q, stream); break;
+      case 40: e = launch_fast<T, 4, 1, false, 0, 1, 64>(P, S, D, Q, stream); break;   // 64 x 4 tiles
+      case 41: e = launch_fast<T, 2, 1, false, 0, 1, 128>(P, S, D, Q, stream); break;  // 128 x 2 tiles
+      case 42: e = launch_fast<T, 4, 2, false, 0, 1, 64>(P, S, D, Q, stream); break;
       case 10: e = launch_stag<T, 8, 1>(P, S, D, Q, stream); break;
       case 11: e = launch_stag<T, 8, 2>(P, S, D, Q, stream); break;
       case 12: e = launch_stag<T, 4, 2>(P, S, D, Q, stream); break;
