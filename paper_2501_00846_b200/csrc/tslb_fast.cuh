@@ -154,35 +154,6 @@ __device__ __forceinline__ Red6<T> reduce6(const T (&v)[3][3]) {   // v[cx+1][cy
   return r;
 }
 
-// ---- cp.async staging of the next source planes (memory pipeline without registers) ---------
-// The kernel is bound by global-memory latency unless several planes per SM are in flight
-// (profiles/r1_ablation.md), and fp64 has no registers to spare for a deeper prefetch.  Each
-// thread therefore copies the 14 scalars of ITS OWN node for plane j+NSTAGE straight into a
-// private shared-memory slot (cp.async, no register staging) and picks them up NSTAGE iterations
-// later; only cp.async.wait_group is needed, no block barrier, because nobody else reads the slot.
-template <typename T, int CELLS>
-struct StageBuf {
-  typename VecOf<T>::type vec[12 / VecOf<T>::W][CELLS];
-  T az[CELLS];
-  T ph[CELLS];
-};
-__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(
-                   (unsigned)__cvta_generic_to_shared(dst)), "l"(src));
-}
-__device__ __forceinline__ void cp_async_small(double* dst, const double* src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(
-                   (unsigned)__cvta_generic_to_shared(dst)), "l"(src));
-}
-__device__ __forceinline__ void cp_async_small(float* dst, const float* src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(
-                   (unsigned)__cvta_generic_to_shared(dst)), "l"(src));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
-}
-
 // ABL != 0 : timing ablations (wrong results on purpose; never selected in production)
 //   bit mask: 1 no shared-memory reads, 2 no closing arithmetic, 4 no global stores,
 //   8 no global loads, 16 no source arithmetic (main warps), 32 no shared-memory writes

@@ -134,12 +134,16 @@ struct K2GatherAll<T, WALLS, TX, TY, 27> {
 template <typename T>
 __device__ __forceinline__ int wrap_plane(int j, int n) { return j < 0 ? j + n : (j >= n ? j - n : j); }
 
-template <typename T, int TX, int TY, bool WALLS, int MINB>
+// NSTAGE = 1: the 14 scalars of the thread's own node for the next plane are fetched with
+// cp.async into a private shared-memory slot while the current plane is processed.
+template <typename T, int TX, int TY, bool WALLS, int MINB, int NSTAGE = 0>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
 k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D, int zchunk) {
   using M = TileMap<TX, TY, 1>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   K2Smem<T, TX, TY>& sm = *reinterpret_cast<K2Smem<T, TX, TY>*>(smem_raw);
+  StageBuf<T, M::CELLS>& stg =
+      *reinterpret_cast<StageBuf<T, M::CELLS>*>(smem_raw + sizeof(K2Smem<T, TX, TY>));
 
   const int tid = threadIdx.x;
   int lx, ly;
@@ -169,6 +173,25 @@ k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ 
   T ph_m = 0, ph_0 = 0, ph_p = 0;    // phi^{n+1} of the own column at planes j-2, j-1, j
   T uo[2][3] = {};                   // u^n of the own node at planes j-1 (slot 0) and j (slot 1)
 
+  auto stage_issue = [&](int j) {
+    if (NSTAGE > 0) {
+      if (in_ring && j <= z1) {
+        using V = typename VecOf<T>::type;
+        int kz2 = 0;
+        const long long s = col + plane * ghost_index(j, P.nz, P.bcz, kz2);
+        cp_async_small(&stg.ph[c], phin + s);
+        if (has_mom && !kz2) {
+          const V* g = reinterpret_cast<const V*>(S);
+#pragma unroll
+          for (int k = 0; k < 12 / VecOf<T>::W; ++k) cp_async16(&stg.vec[k][c], g + k * P.N + s);
+          cp_async_small(&stg.az[c], S + 12 * P.N + s);
+        }
+      }
+      cp_async_commit();
+    }
+  };
+  stage_issue(z0 - 1);
+
   for (int j = z0 - 1; j <= z1; ++j) {
     // ---- source plane j: real, wrapped, or beyond a wall
     int kz = 0;
@@ -178,14 +201,25 @@ k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ 
 
     // phi^{n+1} pipeline (ghost planes mirror evenly, R19)
     ph_m = ph_0; ph_0 = ph_p;
-    if (in_ring) ph_p = phin[col + plane * jz];
+    if (NSTAGE > 0) cp_async_wait<0>();
+    if (in_ring) ph_p = NSTAGE > 0 ? stg.ph[c] : phin[col + plane * jz];
 
     T own[27];
     uo[0][0] = uo[1][0]; uo[0][1] = uo[1][1]; uo[0][2] = uo[1][2];
-    if (has_mom && plane_real) {
-      const long long s = col + plane * jz;
-      T m13[13];
-      load13(S, P.N, s, m13);
+    T m13[13];
+    const bool src_here = has_mom && plane_real;
+    if (src_here) {
+      if (NSTAGE > 0) {
+        constexpr int W = VecOf<T>::W;
+#pragma unroll
+        for (int k = 0; k < 12 / W; ++k) unpack(stg.vec[k][c], &m13[k * W]);
+        m13[12] = stg.az[c];
+      } else {
+        load13(S, P.N, col + plane * jz, m13);
+      }
+    }
+    stage_issue(j + 1);                        // refill the slot just consumed
+    if (src_here) {
       Coef<T> cf = coef_from13(m13);
       uo[1][0] = m13[F_UX]; uo[1][1] = m13[F_UY]; uo[1][2] = m13[F_UZ];
       K2StoreAll<T, TX, TY>::run(sm, c, cf, own);
@@ -223,6 +257,7 @@ k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ 
     }
     __syncthreads();
   }
+  if (NSTAGE > 0) cp_async_wait<0>();
 }
 
 // ------------------------------------------------------------------------------------------
