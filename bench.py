@@ -150,7 +150,7 @@ def run_reference(args):
     glups, dt = time_oracle(cfg, planes, args.steps, args.warmup)
     sample = f"central {nx}x{ny}x{planes} slab of the {nx}^3 input, {args.steps} steps"
     line = {"impl": "reference", "metric": METRIC, "value": glups, "unit": "GLUPS",
-            "n_gpus": 0, "steps": args.steps, "warmup": args.warmup,
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg["name"], "sample": sample},

@@ -45,5 +45,5 @@ def test_reference_arm_is_silent_on_other_ranks(monkeypatch, capsys):
     sys.path.insert(0, ROOT)
     import bench
     monkeypatch.setenv("RANK", "1")
-    bench.run_reference(type("A", (), {"size": 256, "steps": 1, "warmup": 0})())
+    bench.run_reference(type("A", (), {"size": 256, "steps": 1, "warmup": 0, "gpus": 2})())
     assert capsys.readouterr().out == ""
