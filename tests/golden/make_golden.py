@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """Write long-horizon expected values with the CPU ORACLE ONLY (never the CUDA path).
 
-Usage:  python tests/golden/make_golden.py [case ...]      (no argument = every case)
+Usage:  python tests/golden/make_golden.py [--twin] [case ...]   (no case = every case;
+        --twin also records the conditioning run for the large cases, doubling their cost)
 
 For each case the oracle runs the seeded input of paper_2501_00846_b200.inputs for the
 config's full step count and stores, at the checkpoints {1, 10, 100, 1000, ..., final}:
@@ -18,7 +19,7 @@ same inputs through the C ABI and compares.
 Cases (BASELINE.json configs):
   laplace128_R12   configs[1], 128^3, R = 12, 2000 steps               (~1.5 h on 8 cores)
   collision64      configs[3] scaled to 64^3 (R = 6, same We/Re/ratios), 1500 steps
-  bubble48x48x96   configs[2] scaled to 48x48x96 (R = 8, walls in z), 2000 steps
+  bubble32x32x64   configs[2] scaled to 32x32x64 (R = 6, walls in z), 2000 steps
   droplet32        configs[0], 32^3, R = 8, 200 steps
 """
 import os
@@ -42,7 +43,7 @@ def cases():
         "droplet32": (lambda: I.static_droplet(32, 8.0, seed=1), [1, 10, 100, 200]),
         "collision64": (lambda: I.head_on_collision(n=64, radius=6.0, half_sep=10.0),
                         [1, 10, 100, 1000, 1500]),
-        "bubble48x48x96": (lambda: I.rising_bubble(nx=48, ny=48, nz=96, radius=8.0, height=20.0),
+        "bubble32x32x64": (lambda: I.rising_bubble(nx=32, ny=32, nz=64, radius=6.0, height=16.0),
                            [1, 10, 100, 1000, 2000]),
         "laplace128_R12": (lambda: I.static_droplet(128, 12.0, seed=12), [1, 10, 100, 1000, 2000]),
     }
@@ -71,7 +72,7 @@ def run(name):
     sim = R.RefSim(nx, ny, nz, R.make_params(**cfg["params"]))
     sim.init(cfg["phi"], cfg["u"])
     twin = None
-    if nx * ny * nz <= 64 ** 3:                       # conditioning run (small cases only)
+    if nx * ny * nz <= 64 ** 3 or "--twin" in sys.argv:   # conditioning run (costs a second run)
         rng = np.random.Generator(np.random.PCG64(99))
         twin = R.RefSim(nx, ny, nz, R.make_params(**cfg["params"]))
         twin.init(cfg["phi"] * (1.0 + 1e-15 * rng.uniform(-1.0, 1.0, cfg["shape"])), cfg["u"])
@@ -107,5 +108,6 @@ def run(name):
 
 
 if __name__ == "__main__":
-    for nm in (sys.argv[1:] or list(cases())):
+    names = [a for a in sys.argv[1:] if not a.startswith("--")]
+    for nm in (names or list(cases())):
         run(nm)
