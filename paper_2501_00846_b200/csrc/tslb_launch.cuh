@@ -34,12 +34,12 @@ cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStrea
   return cudaGetLastError();
 }
 
-template <typename T, int TY, int MINB>
+template <typename T, int TY, int MINB, int NSTAGE = 0>
 cudaError_t launch_stag(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream) {
   constexpr int TX = 32;
   using M = TileMap<TX, TY, 1>;
-  auto kernel = k_stream_collide_stag<T, TX, TY, MINB>;
-  const size_t smem = sizeof(K2FastSmem<T, M::CELLS>);
+  auto kernel = k_stream_collide_stag<T, TX, TY, MINB, NSTAGE>;
+  const size_t smem = sizeof(K2FastSmem<T, M::CELLS>) + NSTAGE * sizeof(StageBuf<T, M::CELLS>);
   static bool ready = false;
   if (!ready) {
     cudaError_t e = prepare(kernel, smem);
@@ -168,6 +168,9 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
       case 38: e = launch_fast<T, 4, 3, false, 0, 1>(P, S, D, Q, stream); break;
       case 39: e = launch_fast<T, sizeof(T) == 8 ? 8 : 16, 1, false, 0, 2>(P, S, D, Q, stream); break;
       case 40: e = launch_fast<T, 4, 1, false, 0, 1, 64>(P, S, D, Q, stream); break;   // 64 x 4 tiles
+      case 43: e = launch_fast<T, 8, 1, false, 1 + 2 + 16 + 32, 2>(P, S, D, Q, stream); break;  // memory only, 2 stages
+      case 45: e = launch_fast<T, 9, 1, false, 0, 1>(P, S, D, Q, stream); break;
+      case 46: e = launch_fast<T, 6, 1, false, 0, 2>(P, S, D, Q, stream); break;
       case 10: e = launch_stag<T, 8, 1>(P, S, D, Q, stream); break;
       case 11: e = launch_stag<T, 8, 2>(P, S, D, Q, stream); break;
       case 12: e = launch_stag<T, 4, 2>(P, S, D, Q, stream); break;

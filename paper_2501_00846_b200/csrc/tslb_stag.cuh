@@ -19,7 +19,7 @@
 
 namespace tslb {
 
-template <typename T, int TX, int TY, int MINB>
+template <typename T, int TX, int TY, int MINB, int NSTAGE = 0>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
 k_stream_collide_stag(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D,
                       T* __restrict__ Qout, int zchunk) {
@@ -27,6 +27,7 @@ k_stream_collide_stag(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   using SM = K2FastSmem<T, M::CELLS>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
+  StageBuf<T, M::CELLS>& stg = *reinterpret_cast<StageBuf<T, M::CELLS>*>(smem_raw + sizeof(SM));
 
   const int tid = threadIdx.x;
   int lx, ly;
@@ -58,19 +59,45 @@ k_stream_collide_stag(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
     load13(S, P.N, s, m);
     ph = __ldg(phin + s);
   };
-  if (in_ring) load_plane(z0 - 1, nxt, nxt_phi);
+  auto stage_issue = [&](int j) {
+    if (in_ring && j <= z1) {
+      using V = typename VecOf<T>::type;
+      const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
+      const int s = col + plane * jz;
+      const V* g = reinterpret_cast<const V*>(S);
+#pragma unroll
+      for (int k = 0; k < 12 / VecOf<T>::W; ++k) cp_async16(&stg.vec[k][c], g + k * P.N + s);
+      cp_async_small(&stg.az[c], S + 12 * P.N + s);
+      cp_async_small(&stg.ph[c], phin + s);
+    }
+    cp_async_commit();
+  };
+  if (NSTAGE > 0) stage_issue(z0 - 1);
+  else if (in_ring) load_plane(z0 - 1, nxt, nxt_phi);
 
   // ---- S(j): publish plane j into buffer xb, prefetch plane j+1
   auto source = [&](const int j, ExBuf<T, M::CELLS>& xb) {
     ph_a = ph_b; ph_b = ph_c;
 #pragma unroll
     for (int i = 0; i < 3; ++i) { u_a[i] = u_b[i]; u_b[i] = u_c[i]; own_b[i] = own_c[i]; }
+    if (NSTAGE > 0) cp_async_wait<0>();
+    T cur[13];
     if (in_ring) {
-      T cur[13];
+      if (NSTAGE > 0) {
+        constexpr int W = VecOf<T>::W;
 #pragma unroll
-      for (int f = 0; f < 13; ++f) cur[f] = nxt[f];
-      ph_c = nxt_phi;
-      if (j < z1) load_plane(j + 1, nxt, nxt_phi);
+        for (int k = 0; k < 12 / W; ++k) unpack(stg.vec[k][c], &cur[k * W]);
+        cur[12] = stg.az[c];
+        ph_c = stg.ph[c];
+      } else {
+#pragma unroll
+        for (int f = 0; f < 13; ++f) cur[f] = nxt[f];
+        ph_c = nxt_phi;
+        if (j < z1) load_plane(j + 1, nxt, nxt_phi);
+      }
+    }
+    if (NSTAGE > 0) stage_issue(j + 1);
+    if (in_ring) {
       u_c[0] = cur[F_UX]; u_c[1] = cur[F_UY]; u_c[2] = cur[F_UZ];
       const Coef<T> cf = coef_from13(cur);
       SrcFields<T> sf;
@@ -195,6 +222,7 @@ k_stream_collide_stag(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
     iteration(j, acc0, acc1, zo0);
     if (j + 1 <= z1 + 1) iteration(j + 1, acc1, acc0, zo1);
   }
+  if (NSTAGE > 0) cp_async_wait<0>();
 }
 
 }  // namespace tslb

@@ -121,7 +121,7 @@ def test_laplace_128_short_fp64(ref, path):
         assert not bad, (n, bad)
 
 
-@pytest.mark.parametrize("flags", [2, 2 | (1 << 8)] + [v << 8 for v in list(range(13)) + list(range(30, 33)) + list(range(36, 41))] + [v << 16 for v in range(1, 12)])
+@pytest.mark.parametrize("flags", [2, 2 | (1 << 8)] + [v << 8 for v in list(range(13)) + list(range(30, 33)) + list(range(36, 41)) + [45, 46]] + [v << 16 for v in range(1, 12)])
 def test_kernel_variants_fp64(ref, flags):
     """Every tuning variant of the lean periodic kernel (flags bits 8-15) and the wall-capable
     kernel forced onto a periodic box (TSLB_FLAG_GENERIC) meet the same bar."""
