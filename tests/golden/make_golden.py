@@ -1,8 +1,10 @@
 #!/usr/bin/env python
 """Write long-horizon expected values with the CPU ORACLE ONLY (never the CUDA path).
 
-Usage:  python tests/golden/make_golden.py [--twin] [case ...]   (no case = every case;
-        --twin also records the conditioning run for the large cases, doubling their cost)
+Usage:  python tests/golden/make_golden.py [--twin | --twin-only] [case ...]   (no case = every
+        case; --twin also records the conditioning run for the large cases, doubling their cost;
+        --twin-only keeps the stored expected values of an existing file and adds sens_<cp> from
+        one perturbed ORACLE run, measured on the stored sample nodes)
 
 For each case the oracle runs the seeded input of paper_2501_00846_b200.inputs for the
 config's full step count and stores, at the checkpoints {1, 10, 100, 1000, ..., final}:
@@ -107,7 +109,37 @@ def run(name):
     np.savez_compressed(os.path.join(HERE, name + ".npz"), **out)
 
 
+def run_twin_only(name):
+    """Add sens_<cp> to an existing golden file: one perturbed oracle run against the stored
+    sample values (the expected values themselves are left untouched)."""
+    make, checkpoints = cases()[name]
+    path = os.path.join(HERE, name + ".npz")
+    out = dict(np.load(path))
+    cfg = make()
+    nz, ny, nx = cfg["shape"]
+    idx = out["sample_index"]
+    rng = np.random.Generator(np.random.PCG64(99))
+    twin = R.RefSim(nx, ny, nz, R.make_params(**cfg["params"]))
+    twin.init(cfg["phi"] * (1.0 + 1e-15 * rng.uniform(-1.0, 1.0, cfg["shape"])), cfg["u"])
+    done, t0 = 0, time.time()
+    for cp in checkpoints:
+        twin.step(cp - done)
+        done = cp
+        rho, p, u, phi = twin.get()
+        got = (rho.ravel()[idx], p.ravel()[idx], u.reshape(3, -1)[:, idx], phi.ravel()[idx])
+        want = (out[f"rho_{cp}"], out[f"p_{cp}"], out[f"u_{cp}"], out[f"phi_{cp}"])
+        out[f"sens_{cp}"] = np.array([np.abs(a - b).max() / m
+                                      for a, b, m in zip(got, want, out[f"max_{cp}"])])
+        print(f"{name}: twin step {cp} after {time.time() - t0:.0f} s, sens = {out[f'sens_{cp}']}",
+              flush=True)
+        np.savez_compressed(path, **out)
+    twin.close()
+
+
 if __name__ == "__main__":
     names = [a for a in sys.argv[1:] if not a.startswith("--")]
     for nm in (names or list(cases())):
-        run(nm)
+        if "--twin-only" in sys.argv:
+            run_twin_only(nm)
+        else:
+            run(nm)
