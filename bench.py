@@ -301,6 +301,7 @@ def main():
                          "unit": "GB/s", "frac": ach / peak,
                          "traffic": NCU_TRAFFIC.get((prec, dom)) if (periodic_fast and n == 256 ** 3) else None,
                          "peak_kind": peak_kind, "kernel_ms": k_ms,
+                         "kernels_ms": {k: v / args.steps for k, v in r["kernel_ms"].items()},
                          "kernel_share_of_step": r["kernel_ms"][dom] / r["ms"],
                          "algorithmic_bytes_per_update": planes * es,
                          "step_achieved": step_ach, "step_frac": step_ach / peak,

@@ -45,7 +45,7 @@ enum {
   TSLB_FLAG_GENERIC = 2, /* on an all-periodic box, run the wall-capable tiled kernel instead of
                             the lean periodic one (validation of the former at full size)        */
   TSLB_FLAG_VARIANT_MASK = 0xff00 /* bits 8-15: tuning variant of the lean kernel (tile height,
-                            blocks per SM, prefetch), bits 16-19: of the Allen-Cahn kernel;
+                            blocks per SM, prefetch), bits 16-23: of the Allen-Cahn kernel;
                             0 = the production choice                                            */
 };
 

@@ -38,7 +38,7 @@ bool params_ok(int nx, int ny, int nz, const tslb_params* p) {
         p->mobility > 0 && p->sigma >= 0))
     return false;
   if (p->precision != TSLB_F32 && p->precision != TSLB_F64) return false;
-  if (p->flags & ~(TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC | TSLB_FLAG_VARIANT_MASK | 0xf0000)) return false;
+  if (p->flags & ~(TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC | TSLB_FLAG_VARIANT_MASK | 0xff0000)) return false;
   const int n[3] = {nx, ny, nz};
   for (int d = 0; d < 3; ++d) {
     if (p->bc[d] != TSLB_BC_PERIODIC && p->bc[d] != TSLB_BC_WALL) return false;

@@ -259,7 +259,8 @@ __device__ __forceinline__ Coef<T> coef_from13(const T (&m)[13]) {
 // Total Allen-Cahn flux of Eq. 20 at one node (R13, R16):  Q = phi u + kappa_AC phi (1-phi) n,
 // n = grad(phi)/sqrt(|grad(phi)|^2 + eps^2).  The periodic path evaluates it where grad(phi^{n+1})
 // is already known (closing stage of the stream-collide kernel) and stores it for the next
-// step's interface update; layout: plane pair (Qx,Qy) at offset 0, plane Qz at offset 2N.
+// step's interface update; layout: three scalar planes Qx, Qy, Qz at offsets 0, N, 2N (so the
+// interface kernel reads each of them with 128-bit loads, several nodes per thread).
 template <typename T>
 __device__ __forceinline__ void flux_q(const DevParams<T>& P, T phi, T gx, T gy, T gz, T ux, T uy,
                                        T uz, T (&q)[3]) {
@@ -268,21 +269,17 @@ __device__ __forceinline__ void flux_q(const DevParams<T>& P, T phi, T gx, T gy,
   q[1] = fma(phi, uy, s * gy);
   q[2] = fma(phi, uz, s * gz);
 }
-__device__ __forceinline__ void store_q(double* Q, long long N, long long idx, const double (&q)[3]) {
-  reinterpret_cast<double2*>(Q)[idx] = make_double2(q[0], q[1]);
+template <typename T>
+__device__ __forceinline__ void store_q(T* Q, long long N, long long idx, const T (&q)[3]) {
+  Q[idx] = q[0];
+  Q[N + idx] = q[1];
   Q[2 * N + idx] = q[2];
 }
-__device__ __forceinline__ void store_q(float* Q, long long N, long long idx, const float (&q)[3]) {
-  reinterpret_cast<float2*>(Q)[idx] = make_float2(q[0], q[1]);
-  Q[2 * N + idx] = q[2];
-}
-__device__ __forceinline__ void load_q(const double* Q, long long N, long long idx, double (&q)[3]) {
-  const double2 v = __ldg(reinterpret_cast<const double2*>(Q) + idx);
-  q[0] = v.x; q[1] = v.y; q[2] = __ldg(Q + 2 * N + idx);
-}
-__device__ __forceinline__ void load_q(const float* Q, long long N, long long idx, float (&q)[3]) {
-  const float2 v = __ldg(reinterpret_cast<const float2*>(Q) + idx);
-  q[0] = v.x; q[1] = v.y; q[2] = __ldg(Q + 2 * N + idx);
+template <typename T>
+__device__ __forceinline__ void load_q(const T* Q, long long N, long long idx, T (&q)[3]) {
+  q[0] = __ldg(Q + idx);
+  q[1] = __ldg(Q + N + idx);
+  q[2] = __ldg(Q + 2 * N + idx);
 }
 
 // ---- cp.async staging of the next source planes (memory pipeline without registers) ---------

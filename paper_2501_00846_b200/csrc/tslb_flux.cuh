@@ -23,12 +23,7 @@ template <typename T, int CELLS>
 struct FluxBuf { T dv[8][CELLS]; };   // 8 direction scalars (separate arrays: conflict-free reads)
 // cp.async staging slot of one plane: (Qx,Qy), Qz, phi of the thread's own node
 template <typename T, int CELLS>
-struct FluxStage { typename Pair2<T>::type qxy[CELLS]; T qz[CELLS]; T ph[CELLS]; };
-__device__ __forceinline__ void cp_async_pair(double2* dst, const double2* src) { cp_async16(dst, src); }
-__device__ __forceinline__ void cp_async_pair(float2* dst, const float2* src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(
-                   (unsigned)__cvta_generic_to_shared(dst)), "l"(src));
-}
+struct FluxStage { T qx[CELLS]; T qy[CELLS]; T qz[CELLS]; T ph[CELLS]; };
 
 // NSTAGE planes are kept in flight per thread through cp.async (the kernel moves 40 / 20 bytes
 // per update: without a deep memory pipeline it is bound by latency, not bandwidth).
@@ -37,7 +32,6 @@ __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
 k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ Q,
                   T* __restrict__ phin, int zchunk) {
   using M = TileMap<TX, TY, 1>;
-  using P2 = typename Pair2<T>::type;
   extern __shared__ __align__(16) unsigned char flux_smem_raw[];
   FluxBuf<T, M::CELLS>* sm = reinterpret_cast<FluxBuf<T, M::CELLS>*>(flux_smem_raw);
   FluxStage<T, M::CELLS>* stg = reinterpret_cast<FluxStage<T, M::CELLS>*>(
@@ -70,7 +64,8 @@ k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__
     if (in_ring && z <= z1) {
       const int jz = z < 0 ? z + P.nz : (z >= P.nz ? z - P.nz : z);
       const int s = col + plane * jz;
-      cp_async_pair(&stg[slot].qxy[c], reinterpret_cast<const P2*>(Q) + s);
+      cp_async_small(&stg[slot].qx[c], Q + s);
+      cp_async_small(&stg[slot].qy[c], Q + P.N + s);
       cp_async_small(&stg[slot].qz[c], Q + 2 * P.N + s);
       cp_async_small(&stg[slot].ph[c], phi + s);
     }
@@ -103,8 +98,8 @@ k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__
     if (NSTAGE > 0) {
       cp_async_wait<(NSTAGE > 0 ? NSTAGE - 1 : 0)>();   // plane k+1 of the own column has landed
       if (in_ring) {
-        const P2 v = stg[slot].qxy[c];
-        qc[0] = v.x; qc[1] = v.y; qc[2] = stg[slot].qz[c]; fc = stg[slot].ph[c];
+        qc[0] = stg[slot].qx[c]; qc[1] = stg[slot].qy[c]; qc[2] = stg[slot].qz[c];
+        fc = stg[slot].ph[c];
       }
       stage_issue(k + 1 + NSTAGE, slot);
       slot = (slot + 1 == NSTAGE) ? 0 : slot + 1;

@@ -2,6 +2,7 @@
 #pragma once
 #include "tslb_fast.cuh"
 #include "tslb_flux.cuh"
+#include "tslb_flux_row.cuh"
 #include "tslb_stag.cuh"
 #include "tslb_tiled.cuh"
 
@@ -85,6 +86,25 @@ cudaError_t launch_k1_flux(const DevParams<T>& P, const T* S, const T* Q, T* D, 
   return cudaGetLastError();
 }
 
+// row kernel: V = 128 bit / sizeof(T) nodes per thread, zc planes per block
+template <typename T, int TY, int MINB, int NSTAGE>
+cudaError_t launch_k1_row(const DevParams<T>& P, const T* S, const T* Q, T* D, int zc,
+                          cudaStream_t stream) {
+  static_assert(TY + 2 <= 16, "one extra warp owns the 2 (TY + 2) side columns");
+  constexpr int V = RowVec<T>::V;
+  auto kernel = k_allen_cahn_row<T, TY, MINB, NSTAGE>;
+  const size_t smem = sizeof(RowSmem<T, TY, NSTAGE>);
+  static bool ready = false;
+  if (!ready) {
+    cudaError_t e = prepare(kernel, smem);
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  const dim3 grid((P.nx + 32 * V - 1) / (32 * V), (P.ny + TY - 1) / TY, (P.nz + zc - 1) / zc);
+  kernel<<<grid, (TY + 3) * 32, smem, stream>>>(P, S, Q, D + F_PHI * P.N, zc);
+  return cudaGetLastError();
+}
+
 template <typename T, int TY, int MINB, bool WALLS>
 cudaError_t launch_k1w(const DevParams<T>& P, const T* S, T* D, cudaStream_t stream) {
   constexpr int TX = 32;
@@ -116,10 +136,23 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
   const bool generic = walls || (flags & 2);
   const int variant = (flags >> 8) & 0xff;
   cudaError_t e;
-  const int k1v = (flags >> 16) & 0xf;   // bits 16-19: tuning variant of the Allen-Cahn kernel
+  int k1v = (flags >> 16) & 0xff;   // bits 16-23: tuning variant of the Allen-Cahn kernel
   const bool flux_form = !(P.bcx || P.bcy || P.bcz) && !(flags & 2) && (k1v == 0 || k1v >= 5);
+  const bool row_ok = P.nx % RowVec<T>::V == 0;          // vector alignment of every row
+  if (flux_form && k1v == 0) k1v = row_ok ? 20 : 12;     // production choice, periodic
+  if (flux_form && k1v >= 20 && !row_ok) k1v = 12;
   switch (flux_form ? 100 + k1v : k1v) {
-    case 100: e = launch_k1_flux<T, 8, 2, 3>(P, S, Q, D, stream); break;   // production, periodic
+    case 112: e = launch_k1_flux<T, 8, 2, 3>(P, S, Q, D, stream); break;   // one node per thread
+    case 120: e = launch_k1_row<T, 8, 2, 3>(P, S, Q, D, 32, stream); break;   // row kernel
+    case 121: e = launch_k1_row<T, 8, 2, 3>(P, S, Q, D, 16, stream); break;
+    case 122: e = launch_k1_row<T, 8, 2, 3>(P, S, Q, D, 64, stream); break;
+    case 123: e = launch_k1_row<T, 8, 3, 2>(P, S, Q, D, 32, stream); break;
+    case 124: e = launch_k1_row<T, 8, 3, 2>(P, S, Q, D, 16, stream); break;
+    case 125: e = launch_k1_row<T, 12, 2, 2>(P, S, Q, D, 32, stream); break;
+    case 126: e = launch_k1_row<T, 12, 1, 4>(P, S, Q, D, 32, stream); break;
+    case 127: e = launch_k1_row<T, 14, 1, 4>(P, S, Q, D, 32, stream); break;
+    case 128: e = launch_k1_row<T, 4, 4, 3>(P, S, Q, D, 32, stream); break;
+    case 129: e = launch_k1_row<T, 8, 2, 4>(P, S, Q, D, 24, stream); break;
     case 105: e = launch_k1_flux<T, 8, 3, 2>(P, S, Q, D, stream); break;
     case 106: e = launch_k1_flux<T, 8, 3, 4>(P, S, Q, D, stream); break;
     case 107: e = launch_k1_flux<T, 16, 2, 3>(P, S, Q, D, stream); break;

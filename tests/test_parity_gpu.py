@@ -140,6 +140,25 @@ def test_kernel_variants_fp64(ref, flags):
             assert not bad, (flags, prec, n, bad)
 
 
+@pytest.mark.parametrize("k1v", [0, 12] + list(range(20, 30)))
+def test_interface_row_kernel_variants(ref, k1v):
+    """Row kernel of the interface update (several nodes per thread, flags bits 16-23): two x
+    tiles in fp32 (128 + 8 columns), three in fp64 (64 + 64 + 8), ragged in y and z."""
+    cfg, _ = _small_case("ragged_periodic")
+    cfg["shape"] = (36, 19, 136)
+    cfg["phi"] = I.sphere_profile(cfg["shape"], (128.3, 9.1, 16.7), 7.0, 4.0)
+    cfg["u"] = I.noise_u(cfg["shape"], 1e-3, 41)
+    steps = [1, 10]
+    want = run_oracle(ref, cfg, steps)
+    for prec, tol, fields in (("f64", TOL64, ("rho", "p", "u", "phi")), ("f32", TOL32, ("u", "phi"))):
+        got, _ = run_gpu(cfg, steps, prec, k1v << 16)
+        for n, g, r in zip(steps, got, want):
+            errs, bad = compare(ref, cfg, g, r, tol, fields=fields,
+                                state_tol=1e-9 if prec == "f64" else None)
+            print(f"[k1v={k1v} {prec}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+            assert not bad, (k1v, prec, n, bad)
+
+
 def test_host_api_matches_device_api(ref):
     """tslb_init_host / tslb_get_host (the e2e calls of bench.py) give the same fields."""
     cfg, steps = _small_case("bubble_walls_z")
