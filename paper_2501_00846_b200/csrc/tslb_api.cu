@@ -83,6 +83,7 @@ struct tslb_handle {
   int cur;
   bool inited;
   long long launches;
+  tslb::TmaCache tma;     // tensor maps of the two state buffers (TMA-staged kernel)
 };
 
 extern "C" {
@@ -164,7 +165,7 @@ int step_impl(tslb_handle* h, int n, const tslb::Marker& mk) {
       h->launches += 3;
     } else {
       int rc = tslb::launch_step_tiled<T>(P, S, D, reinterpret_cast<T*>(h->scratch), h->stream,
-                                           &h->launches, mk, h->prm.flags);
+                                           &h->launches, mk, h->prm.flags, &h->tma);
       if (rc != 0) return fail(TSLB_ECUDA, "tiled launch: %s", cudaGetErrorString(cudaError_t(rc)));
     }
     h->cur ^= 1;

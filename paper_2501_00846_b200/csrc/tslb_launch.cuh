@@ -1,6 +1,9 @@
 // tslb_launch.cuh -- launch of one time step: kernel selection, grid sizing, attributes.
 #pragma once
+#include <cuda.h>
+
 #include "tslb_fast.cuh"
+#include "tslb_fast_tma.cuh"
 #include "tslb_flux.cuh"
 #include "tslb_flux_row.cuh"
 #include "tslb_stag.cuh"
@@ -20,7 +23,8 @@ inline cudaError_t prepare(K kernel, size_t smem) {
 }
 
 template <typename T, int TY, int MINB, bool PREFETCH, int ABL = 0, int NSTAGE = 0, int TX = 32>
-cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream) {
+cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
+                        int zc = ZCHUNK) {
   using M = TileMap<TX, TY, 1>;
   auto kernel = k_stream_collide_fast<T, TX, TY, MINB, PREFETCH, ABL, NSTAGE>;
   const size_t smem = sizeof(K2FastSmem<T, M::CELLS>) + NSTAGE * sizeof(StageBuf<T, M::CELLS>);
@@ -30,8 +34,97 @@ cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStrea
     if (e != cudaSuccess) return e;
     ready = true;
   }
-  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + ZCHUNK - 1) / ZCHUNK);
-  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, Q, ZCHUNK);
+  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + zc - 1) / zc);
+  kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, Q, zc);
+  return cudaGetLastError();
+}
+
+// ---- TMA-staged lean kernel (tslb_fast_tma.cuh) ---------------------------------------------
+// Tensor maps are encoded through the driver entry point (no link-time dependency on libcuda:
+// the library must load on a machine without a GPU) and cached per source buffer in the handle.
+struct TmaCache {
+  const void* key[2] = {nullptr, nullptr};
+  TmaMaps maps[2];
+};
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+inline EncodeTiledFn tma_encoder() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult st;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &st) == cudaSuccess &&
+        st == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+inline bool tma_encode(TmaMap* out, CUtensorMapDataType dt, int rank, const void* base,
+                       const cuuint64_t* dims, const cuuint64_t* strides, const cuuint32_t* box) {
+  static_assert(sizeof(TmaMap) == sizeof(CUtensorMap), "CUtensorMap is a 128-byte blob");
+  EncodeTiledFn enc = tma_encoder();
+  if (!enc) return false;
+  const cuuint32_t ones[4] = {1, 1, 1, 1};
+  return enc(reinterpret_cast<CUtensorMap*>(out), dt, cuuint32_t(rank), const_cast<void*>(base),
+             dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <typename T, int TX, int TY>
+bool tma_build_maps(const DevParams<T>& P, const T* S, const T* D, TmaMaps* m) {
+  using STG = TmaStage<T, TX, TY>;
+  using M = TileMap<TX, TY, 1>;
+  constexpr int Wel = VecOf<T>::W;
+  const CUtensorMapDataType dt = sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64
+                                                : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+  const cuuint64_t nx = P.nx, ny = P.ny, nz = P.nz, es = sizeof(T);
+  const cuuint64_t vdims[4] = {nx * Wel, ny, nz, cuuint64_t(STG::KV)};
+  const cuuint64_t vstr[3] = {nx * 16, nx * ny * 16, cuuint64_t(P.N) * 16};
+  const cuuint64_t sdims[3] = {nx, ny, nz};
+  const cuuint64_t sstr[2] = {nx * es, nx * ny * es};
+  for (int kind = 0; kind < 4; ++kind) {
+    const bool colw = kind == 1 || kind == 3, roww = kind == 2 || kind == 3;
+    const cuuint32_t vbox[4] = {cuuint32_t((colw ? 1 : M::W) * Wel), cuuint32_t(roww ? 1 : M::HT), 1,
+                                cuuint32_t(STG::KV)};
+    const cuuint32_t sbox[3] = {cuuint32_t(colw ? STG::PAD : STG::PITCH),
+                                cuuint32_t(roww ? 1 : M::HT), 1};
+    if (!tma_encode(&m->vec[kind], dt, 4, S, vdims, vstr, vbox)) return false;
+    if (!tma_encode(&m->az[kind], dt, 3, S + 12 * P.N, sdims, sstr, sbox)) return false;
+    if (!tma_encode(&m->ph[kind], dt, 3, D + F_PHI * P.N, sdims, sstr, sbox)) return false;
+  }
+  return true;
+}
+
+template <typename T> inline bool tma_usable(const DevParams<T>& P) {
+  return P.nx % 32 == 0 && P.nx >= 64 && P.ny > 8;
+}
+
+template <typename T, int TY, int MINB, int NSTAGE>
+cudaError_t launch_tma(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream, int zc,
+                       TmaCache* tc) {
+  constexpr int TX = 32;
+  using M = TileMap<TX, TY, 1>;
+  auto kernel = k_stream_collide_tma<T, TX, TY, MINB, NSTAGE>;
+  constexpr size_t smem = sizeof(K2FastSmem<T, M::CELLS>) + NSTAGE * sizeof(TmaStage<T, TX, TY>) +
+                          NSTAGE * sizeof(unsigned long long);
+  static_assert(smem <= 227 * 1024, "staging depth does not fit in shared memory");
+  static bool ready = false;
+  if (!ready) {
+    cudaError_t e = prepare(kernel, smem);
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  int slot = tc->key[0] == S ? 0 : (tc->key[1] == S ? 1 : -1);
+  if (slot < 0) {
+    slot = tc->key[0] == nullptr ? 0 : 1;
+    if (!tma_build_maps<T, TX, TY>(P, S, D, &tc->maps[slot])) return cudaErrorNotSupported;
+    tc->key[slot] = S;
+  }
+  const dim3 grid(P.nx / TX, (P.ny + TY - 1) / TY, (P.nz + zc - 1) / zc);
+  kernel<<<grid, M::NTHREADS + 32, smem, stream>>>(P, tc->maps[slot], D, Q, zc);
   return cudaGetLastError();
 }
 
@@ -131,7 +224,7 @@ cudaError_t launch_k1(const DevParams<T>& P, const T* S, T* D, cudaStream_t stre
 // variant = (flags >> 8) & 0xff : tuning selector, 0 = production choice.
 template <typename T>
 int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
-                      long long* launches, const Marker& mk, int flags) {
+                      long long* launches, const Marker& mk, int flags, TmaCache* tc = nullptr) {
   const bool walls = P.bcx || P.bcy || P.bcz;
   const bool generic = walls || (flags & 2);
   const int variant = (flags >> 8) & 0xff;
@@ -176,11 +269,49 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
     else
       e = walls ? launch_generic<T, true, NS>(P, S, D, stream) : launch_generic<T, false, NS>(P, S, D, stream);
   } else {
-    switch (variant) {
+    int v2 = variant;
+    if (v2 >= 60 && v2 < 70 && !(tc && tma_usable(P))) v2 = 0;    // TMA staging needs full tile rows
+    switch (v2) {
+      case 60:
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2>(P, S, D, Q, stream, 64, tc);
+        else e = launch_tma<T, 8, 2, 1>(P, S, D, Q, stream, 64, tc);
+        break;
+      case 61:
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 1>(P, S, D, Q, stream, 64, tc);
+        else e = launch_tma<T, 8, 1, 4>(P, S, D, Q, stream, 64, tc);
+        break;
+      case 62:
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2>(P, S, D, Q, stream, 32, tc);
+        else e = launch_tma<T, 8, 2, 1>(P, S, D, Q, stream, 32, tc);
+        break;
       default:   // production choice: fp64 one block/SM, fp32 two blocks/SM
-      case 0:
-        e = sizeof(T) == 8 ? launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream)
-                           : launch_fast<T, 8, 2, false, 0, 1>(P, S, D, Q, stream);
+      case 0: {
+        // 64 planes per block (2 priming planes per chunk instead of 2 per 32) when the grid
+        // still fills the machine about three times over; fp32 then stages two planes ahead
+        constexpr int minb = sizeof(T) == 8 ? 1 : 2;
+        const long long tiles = (long long)((P.nx + 31) / 32) * ((P.ny + 7) / 8);
+        const bool deep = tiles * ((P.nz + 63) / 64) >= 3LL * 148 * minb;
+        if constexpr (sizeof(T) == 8)
+          e = launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream, deep ? 64 : 32);
+        else
+          e = deep ? launch_fast<T, 8, 2, false, 0, 2>(P, S, D, Q, stream, 64)
+                   : launch_fast<T, 8, 2, false, 0, 1>(P, S, D, Q, stream, 32);
+        break;
+      }
+      case 54: e = sizeof(T) == 8 ? launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream, 32)
+                                  : launch_fast<T, 8, 2, false, 0, 1>(P, S, D, Q, stream, 32);
+        break;
+      case 50: e = sizeof(T) == 8 ? launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream, 64)
+                                  : launch_fast<T, 8, 2, false, 0, 1>(P, S, D, Q, stream, 64);
+        break;
+      case 51: e = sizeof(T) == 8 ? launch_fast<T, 8, 1, false, 0, 2>(P, S, D, Q, stream, 64)
+                                  : launch_fast<T, 8, 2, false, 0, 2>(P, S, D, Q, stream, 64);
+        break;
+      case 52: e = sizeof(T) == 8 ? launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream, 128)
+                                  : launch_fast<T, 8, 2, false, 0, 1>(P, S, D, Q, stream, 128);
+        break;
+      case 53: e = sizeof(T) == 8 ? launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream, 43)
+                                  : launch_fast<T, 8, 2, false, 0, 1>(P, S, D, Q, stream, 43);
         break;
       case 6: e = launch_fast<T, 8, 1, false>(P, S, D, Q, stream); break;
       case 7: e = launch_fast<T, 4, 2, false>(P, S, D, Q, stream); break;

@@ -121,7 +121,7 @@ def test_laplace_128_short_fp64(ref, path):
         assert not bad, (n, bad)
 
 
-@pytest.mark.parametrize("flags", [2, 2 | (1 << 8)] + [v << 8 for v in list(range(13)) + list(range(30, 33)) + list(range(36, 41)) + [45, 46]] + [v << 16 for v in range(1, 12)])
+@pytest.mark.parametrize("flags", [2, 2 | (1 << 8)] + [v << 8 for v in list(range(13)) + list(range(30, 33)) + list(range(36, 41)) + [45, 46, 50, 51, 54]] + [v << 16 for v in range(1, 12)])
 def test_kernel_variants_fp64(ref, flags):
     """Every tuning variant of the lean periodic kernel (flags bits 8-15) and the wall-capable
     kernel forced onto a periodic box (TSLB_FLAG_GENERIC) meet the same bar."""
@@ -157,6 +157,25 @@ def test_interface_row_kernel_variants(ref, k1v):
                                 state_tol=1e-9 if prec == "f64" else None)
             print(f"[k1v={k1v} {prec}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
             assert not bad, (k1v, prec, n, bad)
+
+
+@pytest.mark.parametrize("nx,variant", [(96, 60), (96, 61), (64, 62), (128, 60)])
+def test_tma_staged_kernel(ref, nx, variant):
+    """Stream-collide kernel with TMA bulk staging (flags bits 8-15 = 60, 62; kept as a measured, rejected variant): x tiles that wrap
+    on the left, on the right, on both sides (nx = 32) and not at all; ragged in y and z."""
+    cfg, _ = _small_case("ragged_periodic")
+    cfg["shape"] = (70, 19, nx)
+    cfg["phi"] = I.sphere_profile(cfg["shape"], (nx - 2.7, 9.1, 30.7), 7.0, 4.0)
+    cfg["u"] = I.noise_u(cfg["shape"], 1e-3, 43)
+    steps = [1, 10]
+    want = run_oracle(ref, cfg, steps)
+    for prec, tol, fields in (("f64", TOL64, ("rho", "p", "u", "phi")), ("f32", TOL32, ("u", "phi"))):
+        got, _ = run_gpu(cfg, steps, prec, variant << 8)
+        for n, g, r in zip(steps, got, want):
+            errs, bad = compare(ref, cfg, g, r, tol, fields=fields,
+                                state_tol=1e-9 if prec == "f64" else None)
+            print(f"[nx={nx} v={variant} {prec}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+            assert not bad, (nx, variant, prec, n, bad)
 
 
 def test_host_api_matches_device_api(ref):
