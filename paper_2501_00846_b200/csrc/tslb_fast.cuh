@@ -22,12 +22,15 @@ __host__ __device__ constexpr int dir_slot(int cx, int cy) {
 }
 
 // Exchange buffers, double buffered over the marching index so that one __syncthreads per plane
-// is enough.  Per direction and cell: (E,O) as one pair word (128 bit in fp64, 64 bit in fp32)
-// and Qq as a scalar; every access is contiguous across the warp (no bank conflicts).
-template <typename T, int CELLS> struct ExBuf;
-template <int CELLS> struct ExBuf<double, CELLS> {
-  double2 eo[8][CELLS];
-  double q[8][CELLS];
+// is enough.  Per direction: (E,O) as one pair word (128 bit in fp64, 64 bit in fp32) and Qq as a
+// scalar, indexed by the RECEIVER (main thread index ly TX + lx): a source writes direction
+// (cx,cy) at its own index + cy TX + cx, and only if that node lies inside the tile, so ring
+// cells and tile-edge cells skip the directions nobody reads; a receiver finds all 8 arrivals at
+// its own index.  Every access is contiguous across the warp (no bank conflicts).
+template <typename T, int CELLS, int NMAIN> struct ExBuf;
+template <int CELLS, int NMAIN> struct ExBuf<double, CELLS, NMAIN> {
+  double2 eo[8][NMAIN];
+  double q[8][NMAIN];
   double2 pd[CELLS];      // (pz, dz) of phi^{n+1}: (phi(z-1)+phi(z+1)) + 4 phi(z),  phi(z+1) - phi(z-1)
   __device__ __forceinline__ void put(int slot, int c, double E, double O, double Q) {
     eo[slot][c] = make_double2(E, O);
@@ -46,9 +49,9 @@ template <int CELLS> struct ExBuf<double, CELLS> {
     const double2 v = pd[c]; a = v.x; b = v.y;
   }
 };
-template <int CELLS> struct ExBuf<float, CELLS> {
-  float2 eo[8][CELLS];
-  float q[8][CELLS];
+template <int CELLS, int NMAIN> struct ExBuf<float, CELLS, NMAIN> {
+  float2 eo[8][NMAIN];
+  float q[8][NMAIN];
   float2 pd[CELLS];
   __device__ __forceinline__ void put(int slot, int c, float E, float O, float Q) {
     eo[slot][c] = make_float2(E, O);
@@ -67,8 +70,22 @@ template <int CELLS> struct ExBuf<float, CELLS> {
     const float2 v = pd[c]; a = v.x; b = v.y;
   }
 };
-template <typename T, int CELLS>
-struct K2FastSmem { ExBuf<T, CELLS> buf[2]; };
+template <typename T, int CELLS, int NMAIN>
+struct K2FastSmem { ExBuf<T, CELLS, NMAIN> buf[2]; };
+
+// which of the 8 in-plane directions of the ring cell (lx, ly) have their receiver inside the tile
+template <int TX, int TY>
+__device__ __forceinline__ unsigned dir_mask(int lx, int ly) {
+  unsigned m = 0;
+#pragma unroll
+  for (int q = 0; q < 9; ++q) {
+    const int cx = q % 3 - 1, cy = q / 3 - 1;
+    if (cx == 0 && cy == 0) continue;
+    const int rx = lx + cx, ry = ly + cy;
+    if (rx >= 0 && rx < TX && ry >= 0 && ry < TY) m |= 1u << dir_slot(cx, cy);
+  }
+  return m;
+}
 
 // E, O, Qq on the 3x3 in-plane directions, index [cx+1][cy+1], all scaled by 1/216.
 template <typename T> struct SrcFields { T E[3][3], O[3][3], Q[3][3]; };
@@ -163,7 +180,8 @@ __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
 k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D,
                       T* __restrict__ Qout, int zchunk) {
   using M = TileMap<TX, TY, 1>;
-  using SM = K2FastSmem<T, M::CELLS>;
+  using SM = K2FastSmem<T, M::CELLS, M::NMAIN>;
+  using XB = ExBuf<T, M::CELLS, M::NMAIN>;
   using STG = StageBuf<T, M::CELLS>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
@@ -177,6 +195,8 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   const int z0 = blockIdx.z * zchunk;
   const int z1 = min(P.nz, z0 + zchunk);
   const int c = M::cell(lx, ly);
+  const int rb = ly * TX + lx;                                  // index as a receiver (main: tid)
+  const unsigned need = mapped ? dir_mask<TX, TY>(lx, ly) : 0u; // directions somebody reads
   const bool in_ring = mapped && gx >= -1 && gx <= P.nx && gy >= -1 && gy <= P.ny;
   const bool is_out = tid < M::NMAIN && gx < P.nx && gy < P.ny;
   const int sx = gx < 0 ? gx + P.nx : (gx >= P.nx ? gx - P.nx : gx);      // periodic wrap
@@ -248,7 +268,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
       load_plane(z0, pb, fb);
     }
     for (int j = z0 - 1; j <= z1; ++j) {
-      ExBuf<T, M::CELLS>& xb = sm.buf[(j - z0 + 1) & 1];
+      XB& xb = sm.buf[(j - z0 + 1) & 1];
       ph_m = ph_0; ph_0 = ph_p;
       if (in_ring) {
         T cur[13];
@@ -263,7 +283,8 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         for (int q = 0; q < 9; ++q) {
           const int cx = q % 3 - 1, cy = q / 3 - 1;
           if (cx == 0 && cy == 0) continue;
-          xb.put(dir_slot(cx, cy), c, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
+          if (need >> dir_slot(cx, cy) & 1u)
+            xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
         }
         xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
       }
@@ -273,7 +294,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   }
   if (REGPF && in_ring) load_plane(z0 - 1, nxt, nxt_phi);
 
-  auto body = [&](const int j, const int slot, ExBuf<T, M::CELLS>& xb, T (&aA)[6], T (&aB)[6],
+  auto body = [&](const int j, const int slot, XB& xb, T (&aA)[6], T (&aB)[6],
                   T (&zA)[3], T (&zB)[3], const T (&uPrev)[3], T (&uCur)[3]) {
     T ownE = 0, ownO = 0, ownQ = 0;
     ph_m = ph_0; ph_0 = ph_p;
@@ -303,7 +324,8 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
       for (int q = 0; q < 9; ++q) {
         const int cx = q % 3 - 1, cy = q / 3 - 1;
         if (cx == 0 && cy == 0) continue;
-        if (!(ABL & 32) || cx + cy == 2) xb.put(dir_slot(cx, cy), c, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
+        if ((need >> dir_slot(cx, cy) & 1u) && (!(ABL & 32) || cx + cy == 2))
+          xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
       }
       xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
     }
@@ -321,7 +343,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
           const int cx = q % 3 - 1, cy = q / 3 - 1;
           if (cx == 0 && cy == 0) continue;
           if ((ABL & 1) && q != 8) { vE[cx + 1][cy + 1] = ownE * T(q); vO[cx + 1][cy + 1] = ownO * T(q); continue; }
-          xb.get_eo(dir_slot(cx, cy), c - cy * M::W - cx, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
+          xb.get_eo(dir_slot(cx, cy), tid, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
         }
         rE = reduce6(vE);
         rO = reduce6(vO);
@@ -335,7 +357,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
           const int cx = q % 3 - 1, cy = q / 3 - 1;
           if (cx == 0 && cy == 0) continue;
           if ((ABL & 1) && q != 8) { vQ[cx + 1][cy + 1] = ownQ * T(q); continue; }
-          xb.get_q(dir_slot(cx, cy), c - cy * M::W - cx, vQ[cx + 1][cy + 1]);
+          xb.get_q(dir_slot(cx, cy), tid, vQ[cx + 1][cy + 1]);
         }
         rQ = reduce6(vQ);
       }

@@ -107,7 +107,8 @@ __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS + 32), MINB)
 k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __restrict__ D,
                      T* __restrict__ Qout, int zchunk) {
   using M = TileMap<TX, TY, 1>;
-  using SM = K2FastSmem<T, M::CELLS>;
+  using SM = K2FastSmem<T, M::CELLS, M::NMAIN>;
+  using XB = ExBuf<T, M::CELLS, M::NMAIN>;
   using STG = TmaStage<T, TX, TY>;
   using V = typename VecOf<T>::type;
   constexpr int W = VecOf<T>::W;
@@ -190,6 +191,8 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
   const bool mapped = M::coords(tid, lx, ly);
   const int gx = gx0 + lx, gy = gy0 + ly;
   const int c = M::cell(lx, ly);
+  const int rb = ly * TX + lx;                                  // index as a receiver (main: tid)
+  const unsigned need = mapped ? dir_mask<TX, TY>(lx, ly) : 0u; // directions somebody reads
   const bool in_ring = mapped && gy >= -1 && gy <= P.ny;            // nx % TX == 0: x always in
   const bool is_out = tid < M::NMAIN && gy < P.ny;
   // where this thread's node lands in a staging slot (byte offsets from the slot base)
@@ -220,7 +223,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
   T acc0[6] = {}, acc1[6] = {}, zo0[3] = {}, zo1[3] = {}, u0[3] = {}, u1[3] = {};
   T ph_m = 0, ph_0 = 0, ph_p = 0;
 
-  auto body = [&](const int j, const int slot, const unsigned parity, ExBuf<T, M::CELLS>& xb,
+  auto body = [&](const int j, const int slot, const unsigned parity, XB& xb,
                   T (&aA)[6], T (&aB)[6], T (&zA)[3], T (&zB)[3], const T (&uPrev)[3],
                   T (&uCur)[3]) {
     T ownE = 0, ownO = 0, ownQ = 0;
@@ -243,7 +246,8 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
       for (int q = 0; q < 9; ++q) {
         const int cx = q % 3 - 1, cy = q / 3 - 1;
         if (cx == 0 && cy == 0) continue;
-        xb.put(dir_slot(cx, cy), c, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
+        if (need >> dir_slot(cx, cy) & 1u)
+          xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
       }
       xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
     }
@@ -258,7 +262,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
         for (int q = 0; q < 9; ++q) {
           const int cx = q % 3 - 1, cy = q / 3 - 1;
           if (cx == 0 && cy == 0) continue;
-          xb.get_eo(dir_slot(cx, cy), c - cy * M::W - cx, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
+          xb.get_eo(dir_slot(cx, cy), tid, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
         }
         rE = reduce6(vE);
         rO = reduce6(vO);
@@ -271,7 +275,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
         for (int q = 0; q < 9; ++q) {
           const int cx = q % 3 - 1, cy = q / 3 - 1;
           if (cx == 0 && cy == 0) continue;
-          xb.get_q(dir_slot(cx, cy), c - cy * M::W - cx, vQ[cx + 1][cy + 1]);
+          xb.get_q(dir_slot(cx, cy), tid, vQ[cx + 1][cy + 1]);
         }
         rQ = reduce6(vQ);
       }

@@ -121,7 +121,7 @@ def test_laplace_128_short_fp64(ref, path):
         assert not bad, (n, bad)
 
 
-@pytest.mark.parametrize("flags", [2, 2 | (1 << 8)] + [v << 8 for v in list(range(13)) + list(range(30, 33)) + list(range(36, 41)) + [45, 46, 50, 51, 54]] + [v << 16 for v in range(1, 12)])
+@pytest.mark.parametrize("flags", [2, 2 | (1 << 8)] + [v << 8 for v in list(range(13)) + list(range(30, 33)) + list(range(36, 41)) + [45, 46, 50, 51, 54, 55, 56]] + [v << 16 for v in range(1, 12)])
 def test_kernel_variants_fp64(ref, flags):
     """Every tuning variant of the lean periodic kernel (flags bits 8-15) and the wall-capable
     kernel forced onto a periodic box (TSLB_FLAG_GENERIC) meet the same bar."""
@@ -159,7 +159,7 @@ def test_interface_row_kernel_variants(ref, k1v):
             assert not bad, (k1v, prec, n, bad)
 
 
-@pytest.mark.parametrize("nx,variant", [(96, 60), (96, 61), (64, 62), (128, 60)])
+@pytest.mark.parametrize("nx,variant", [(96, 60), (96, 61), (64, 62), (128, 60), (96, 70), (64, 71), (128, 72)])
 def test_tma_staged_kernel(ref, nx, variant):
     """Stream-collide kernel with TMA bulk staging (flags bits 8-15 = 60, 62; kept as a measured, rejected variant): x tiles that wrap
     on the left, on the right, on both sides (nx = 32) and not at all; ragged in y and z."""
