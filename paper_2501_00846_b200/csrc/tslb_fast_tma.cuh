@@ -102,7 +102,10 @@ struct TmaStage {
   static constexpr unsigned B_WXY = KV * 16 + 2 * 16;
 };
 
-template <typename T, int TX, int TY, int MINB, int NSTAGE>
+// ABL != 0 : timing ablation (wrong results on purpose; never selected in production)
+//   1 = memory only: every thread takes its node from the staging slot and the main threads store
+//       14 + 3 scalars derived from it by a few additions; no reconstruction, exchange or closing
+template <typename T, int TX, int TY, int MINB, int NSTAGE, int ABL = 0>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS + 32), MINB)
 k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __restrict__ D,
                      T* __restrict__ Qout, int zchunk) {
@@ -227,6 +230,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
                   T (&aA)[6], T (&aB)[6], T (&zA)[3], T (&zB)[3], const T (&uPrev)[3],
                   T (&uCur)[3]) {
     T ownE = 0, ownO = 0, ownQ = 0;
+    T abl[13] = {};
     ph_m = ph_0; ph_0 = ph_p;
     mbar_wait(&full[slot], parity);                    // plane j has landed
     if (in_ring) {
@@ -237,6 +241,11 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
         unpack(*reinterpret_cast<const V*>(sb + voff + k * vstride), &cur[k * W]);
       cur[12] = *reinterpret_cast<const T*>(sb + azoff);
       ph_p = *reinterpret_cast<const T*>(sb + phoff);
+      if (ABL & 1) {
+        abl[0] = cur[0] + ph_p;
+#pragma unroll
+        for (int f = 1; f < 13; ++f) abl[f] = cur[f];
+      } else {
       uCur[0] = cur[F_UX]; uCur[1] = cur[F_UY]; uCur[2] = cur[F_UZ];
       SrcFields<T> sf;
       const Coef<T> cf = coef_from13(cur);
@@ -250,8 +259,23 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
           xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
       }
       xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
+      }
     }
     __syncthreads();
+    if (ABL & 1) {
+      if (is_out && j - 1 >= z0) {
+        NodeOut<T> out;
+        out.p = abl[0]; out.ux = abl[1]; out.uy = abl[2]; out.uz = abl[3];
+        out.axx = abl[4]; out.ayy = abl[5]; out.azz = abl[6]; out.axy = abl[7];
+        out.axz = abl[8]; out.ayz = abl[9]; out.ax = abl[10]; out.ay = abl[11]; out.az = abl[12];
+        const long long idx = gx + P.nx * gy + (long long)plane * (j - 1);
+        store_out(D, P.N, idx, out);
+        T q[3] = {abl[1] + ph_p, abl[2] + ph_p, abl[3] + ph_p};
+        store_q(Qout, P.N, idx, q);
+      }
+      return;
+    }
+
 
     if (is_out) {
       Red6<T> rE, rO, rQ;
