@@ -36,7 +36,10 @@ def parse():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--size", type=int, default=256, help="cube edge of the collision domain")
+    ap.add_argument("--size", type=int, default=256, help="cube edge of the domain")
+    ap.add_argument("--workload", default="collision", choices=["collision", "emulsion"],
+                    help="collision = BASELINE.json configs[3] (the graded one); emulsion = "
+                         "configs[4], the throughput sweep (use --size 384 for f64, 512 for f32)")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
                     help="precision of the headline value (the other one is reported beside it)")
     ap.add_argument("--naive", action="store_true", help="time the validation kernels instead")
@@ -104,8 +107,10 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
-def make_workload(size):
+def make_workload(size, kind="collision"):
     from paper_2501_00846_b200 import inputs as I
+    if kind == "emulsion":
+        return I.emulsion_sweep(n=size)
     s = size / 256.0
     return I.head_on_collision(n=size, radius=24.0 * s, half_sep=40.0 * s)
 
@@ -141,7 +146,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cfg = make_workload(args.size)
+    cfg = make_workload(args.size, args.workload)
     nz, ny, nx = cfg["shape"]
     rate, _ = time_oracle(cfg, 4, 1)                      # calibration: 4 planes, 1 step
     budget = 100.0                                         # seconds for warmup + steps
@@ -275,7 +280,7 @@ def main():
     barrier, max_over_ranks = ranks.barrier, ranks.max
 
     flags = (1 if args.naive else 0) | (2 if args.generic else 0) | (args.variant << 8) | (args.k1variant << 16)
-    cfg = make_workload(args.size)
+    cfg = make_workload(args.size, args.workload)
     n = int(np.prod(cfg["shape"]))
     peak, peak_kind = peaks()
     order = [args.only] if args.only else [args.precision, "f32" if args.precision == "f64" else "f64"]
@@ -325,7 +330,8 @@ def main():
                 "ms_per_step": head["ms"] / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": order[0], "data": "synthetic",
                 "config": {"workload": cfg["name"], "grid": list(cfg["shape"][::-1]),
-                           "parallelism": f"replicas x{world}", "l2": "state 3.8 GB (f64) >> L2",
+                           "parallelism": f"replicas x{world}",
+                           "l2": f"state {2 * STATE_SCALARS * (8 if order[0] == 'f64' else 4) * n / 1e9:.1f} GB ({order[0]}) >> 126 MB L2",
                            "path": "naive" if args.naive else ("tiled-generic" if args.generic else "tiled"),
                            "variant": args.variant},
                 "clocks": head["clocks"], "gpu_launches": head["launches"],
