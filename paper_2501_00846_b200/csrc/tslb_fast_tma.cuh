@@ -74,6 +74,19 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const TmaMap* map, int c0
       : "memory");
 }
 
+// L2 prefetch of a box (no shared memory involved): the DRAM access of a plane that will be staged
+// NSTAGE + PF iterations from now starts early, so the staging copy itself finds the data in L2
+__device__ __forceinline__ void tma_prefetch_4d(const TmaMap* map, int c0, int c1, int c2, int c3) {
+  asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global [%0, {%1, %2, %3, %4}];" ::"l"(map),
+               "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+               : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_3d(const TmaMap* map, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global [%0, {%1, %2, %3}];" ::"l"(map),
+               "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+
 // staging slot of one source plane: the ring of the tile, all 14 scalars.  Out-of-range parts of
 // the main boxes are zero-filled by the TMA unit; the periodic images land in the w* arrays and
 // the threads on a wrapped column / row read those instead.
@@ -105,7 +118,8 @@ struct TmaStage {
 // ABL != 0 : timing ablation (wrong results on purpose; never selected in production)
 //   1 = memory only: every thread takes its node from the staging slot and the main threads store
 //       14 + 3 scalars derived from it by a few additions; no reconstruction, exchange or closing
-template <typename T, int TX, int TY, int MINB, int NSTAGE, int ABL = 0>
+// PF > 0 : the producer also prefetches the main boxes of plane j + NSTAGE + PF into L2
+template <typename T, int TX, int TY, int MINB, int NSTAGE, int ABL = 0, int PF = 0>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS + 32), MINB)
 k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __restrict__ D,
                      T* __restrict__ Qout, int zchunk) {
@@ -149,6 +163,11 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
     const int ys_w = yw_b ? P.ny - 1 : 0;                      // source row of the wrapped row
     auto produce = [&](int j, int slot) {
       if (j > z1) return;
+      if (PF > 0 && lane >= 16 && lane < 19 && j + PF <= z1) {   // L2 prefetch, main boxes only
+        const int jp = j + PF >= P.nz ? j + PF - P.nz : (j + PF < 0 ? j + PF + P.nz : j + PF);
+        if (lane == 16) tma_prefetch_4d(&maps.vec[0], (gx0 - 1) * W, gy0 - 1, jp, 0);
+        else tma_prefetch_3d(lane == 17 ? &maps.az[0] : &maps.ph[0], gx0 - STG::PAD, gy0 - 1, jp);
+      }
       const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
       STG& st = stg[slot];
       unsigned long long* bar = &full[slot];

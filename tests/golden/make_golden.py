@@ -1,10 +1,13 @@
 #!/usr/bin/env python
 """Write long-horizon expected values with the CPU ORACLE ONLY (never the CUDA path).
 
-Usage:  python tests/golden/make_golden.py [--twin | --twin-only] [case ...]   (no case = every
-        case; --twin also records the conditioning run for the large cases, doubling their cost;
-        --twin-only keeps the stored expected values of an existing file and adds sens_<cp> from
-        one perturbed ORACLE run, measured on the stored sample nodes)
+Usage:  python tests/golden/make_golden.py [--twin | --twin-only [--perturb-u]] [case ...]
+        (no case = every case; --twin also records the conditioning run for the large cases,
+        doubling their cost; --twin-only keeps the stored expected values of an existing file and
+        adds sens_<cp> from one perturbed ORACLE run, measured on the stored sample nodes;
+        --perturb-u also perturbs the input velocity by 1e-21 (absolute, the size of the
+        one-step rounding differences between two summation orders), which reaches the gas
+        phase where a relative perturbation of phi ~ 1e-9 is no perturbation at all)
 
 For each case the oracle runs the seeded input of paper_2501_00846_b200.inputs for the
 config's full step count and stores, at the checkpoints {1, 10, 100, 1000, ..., final}:
@@ -120,7 +123,12 @@ def run_twin_only(name):
     idx = out["sample_index"]
     rng = np.random.Generator(np.random.PCG64(99))
     twin = R.RefSim(nx, ny, nz, R.make_params(**cfg["params"]))
-    twin.init(cfg["phi"] * (1.0 + 1e-15 * rng.uniform(-1.0, 1.0, cfg["shape"])), cfg["u"])
+    phi0 = cfg["phi"] * (1.0 + 1e-15 * rng.uniform(-1.0, 1.0, cfg["shape"]))
+    u0 = cfg["u"]
+    if "--perturb-u" in sys.argv:
+        u0 = u0 + 1e-21 * rng.uniform(-1.0, 1.0, u0.shape)
+        out["sens_perturb_u"] = np.array(1e-21)
+    twin.init(phi0, u0)
     done, t0 = 0, time.time()
     for cp in checkpoints:
         twin.step(cp - done)
