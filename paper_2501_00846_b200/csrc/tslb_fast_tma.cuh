@@ -7,9 +7,10 @@
 // population exchange already loads to ~60 % (profiles/r1b_*).  Here ONE extra warp issues
 // cp.async.bulk.tensor copies (TMA) for the whole ring of the tile, NSTAGE planes ahead,
 // completing on an mbarrier per staging slot:
-//   * one 4-d box (x, y, z, f) brings all 128-bit field-vector planes of the ring, one 3-d box
-//     each the scalar planes az and phi^{n+1} (staged with a 16-byte pad on both sides of a row so
-//     that the box is 16-byte granular): 3 copies per plane for an interior tile;
+//   * one 4-d box (x, y, z, f) per 128-bit field-vector plane of the ring (SPLIT, production:
+//     6 boxes in fp64; a single box for all planes is 4.5 % slower), one 3-d box each for the
+//     scalar planes az and phi^{n+1} (staged with a 16-byte pad on both sides of a row so that
+//     the box is 16-byte granular): 8 copies per plane for an interior tile in fp64;
 //   * the parts of a box beyond the lattice are zero-filled by the TMA unit; the periodic images
 //     (one column, one row, one corner cell at most) come with up to 9 small extra boxes into
 //     separate arrays, and the threads of a wrapped column / row read those instead;
@@ -55,7 +56,7 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
 // Each exists with four box shapes: the whole ring (main), one wrapped column (wx), one wrapped
 // row (wy), one wrapped corner cell (wxy).  128-byte opaque blobs (CUtensorMap).
 struct alignas(64) TmaMap { unsigned long long opaque[16]; };
-struct TmaMaps { TmaMap vec[4], az[4], ph[4]; };      // [main, wx, wy, wxy]
+struct TmaMaps { TmaMap vec[4], az[4], ph[4], vecf; };   // [main, wx, wy, wxy]; vecf: one field plane of main
 
 __device__ __forceinline__ void tma_load_4d(void* dst, const TmaMap* map, int c0, int c1, int c2,
                                             int c3, unsigned long long* bar) {
@@ -90,14 +91,16 @@ __device__ __forceinline__ void tma_prefetch_3d(const TmaMap* map, int c0, int c
 // staging slot of one source plane: the ring of the tile, all 14 scalars.  Out-of-range parts of
 // the main boxes are zero-filled by the TMA unit; the periodic images land in the w* arrays and
 // the threads on a wrapped column / row read those instead.
-template <typename T, int TX, int TY>
+template <typename T, int TX, int TY, bool PADDED = false>
 struct TmaStage {
   using M = TileMap<TX, TY, 1>;
+  // cells per field plane: padded to a multiple of 128 bytes when every plane is its own box
+  static constexpr int VP = PADDED ? (TileMap<TX, TY, 1>::CELLS + 7) / 8 * 8 : TileMap<TX, TY, 1>::CELLS;
   using V = typename VecOf<T>::type;
   static constexpr int KV = 12 / VecOf<T>::W;          // 128-bit field-vector planes
   static constexpr int PAD = 16 / int(sizeof(T));      // scalars in 16 bytes
   static constexpr int PITCH = TX + 2 * PAD;
-  alignas(128) V vec[KV][M::CELLS];                    // box (W, HT, 1, KV)
+  alignas(128) V vec[KV][VP];                          // box (W, HT, 1, KV)
   alignas(128) V vwx[KV][M::HT];                       // box (1, HT, 1, KV)
   alignas(128) V vwy[KV][M::W];                        // box (W, 1, 1, KV)
   alignas(128) V vwxy[KV];                             // box (1, 1, 1, KV)
@@ -118,15 +121,17 @@ struct TmaStage {
 // ABL != 0 : timing ablation (wrong results on purpose; never selected in production)
 //   1 = memory only: every thread takes its node from the staging slot and the main threads store
 //       14 + 3 scalars derived from it by a few additions; no reconstruction, exchange or closing
+//   1 + 2 = loads only (one store per thread at the end), 1 + 4 = stores only (no TMA traffic)
 // PF > 0 : the producer also prefetches the main boxes of plane j + NSTAGE + PF into L2
-template <typename T, int TX, int TY, int MINB, int NSTAGE, int ABL = 0, int PF = 0>
+// SPLIT  : the main field-vector box is issued as KV boxes of one field plane each
+template <typename T, int TX, int TY, int MINB, int NSTAGE, int ABL = 0, int PF = 0, bool SPLIT = false>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS + 32), MINB)
 k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __restrict__ D,
                      T* __restrict__ Qout, int zchunk) {
   using M = TileMap<TX, TY, 1>;
   using SM = K2FastSmem<T, M::CELLS, M::NMAIN>;
   using XB = ExBuf<T, M::CELLS, M::NMAIN>;
-  using STG = TmaStage<T, TX, TY>;
+  using STG = TmaStage<T, TX, TY, SPLIT>;
   using V = typename VecOf<T>::type;
   constexpr int W = VecOf<T>::W;
   extern __shared__ __align__(128) unsigned char tma_smem_raw[];
@@ -162,7 +167,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
     const int xsa_w = xw_l ? P.nx - STG::PAD : 0;              // ... of the 16-byte scalar group
     const int ys_w = yw_b ? P.ny - 1 : 0;                      // source row of the wrapped row
     auto produce = [&](int j, int slot) {
-      if (j > z1) return;
+      if (j > z1 || (ABL & 4)) return;
       if (PF > 0 && lane >= 16 && lane < 19 && j + PF <= z1) {   // L2 prefetch, main boxes only
         const int jp = j + PF >= P.nz ? j + PF - P.nz : (j + PF < 0 ? j + PF + P.nz : j + PF);
         if (lane == 16) tma_prefetch_4d(&maps.vec[0], (gx0 - 1) * W, gy0 - 1, jp, 0);
@@ -174,6 +179,9 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
       if (lane == 0) mbar_expect_tx(bar, bytes);
       __syncwarp();
       const int kind = lane / 3, what = lane % 3;              // kind: main, wx, wy, wxy
+      if (SPLIT && lane >= 20 && lane < 20 + STG::KV)
+        tma_load_4d(&st.vec[lane - 20][0], &maps.vecf, (gx0 - 1) * W, gy0 - 1, jz, lane - 20, bar);
+      if (SPLIT && lane == 0) return;
       if (lane >= 12) return;
       if (kind == 1 && !xw) return;
       if (kind == 2 && !yw) return;
@@ -224,7 +232,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
     const bool yw = (yw_b || yw_t) && ly + 1 == r_w;
     const int r = ly + 1, xa = lx == -1 ? STG::PAD - 1 : 0;          // scalar inside its 16-byte group
     if (!xw && !yw) {
-      voff = offsetof(STG, vec) + c * 16; vstride = M::CELLS * 16;
+      voff = offsetof(STG, vec) + c * 16; vstride = STG::VP * 16;
       azoff = offsetof(STG, az) + (r * STG::PITCH + lx + STG::PAD) * sizeof(T);
       phoff = offsetof(STG, ph) + (r * STG::PITCH + lx + STG::PAD) * sizeof(T);
     } else if (xw && !yw) {
@@ -251,7 +259,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
     T ownE = 0, ownO = 0, ownQ = 0;
     T abl[13] = {};
     ph_m = ph_0; ph_0 = ph_p;
-    mbar_wait(&full[slot], parity);                    // plane j has landed
+    if (!(ABL & 4)) mbar_wait(&full[slot], parity);    // plane j has landed
     if (in_ring) {
       T cur[13];
       const unsigned char* sb = reinterpret_cast<const unsigned char*>(&stg[slot]);
@@ -282,7 +290,11 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
     }
     __syncthreads();
     if (ABL & 1) {
-      if (is_out && j - 1 >= z0) {
+      if (ABL & 2) {                                   // loads only: keep the values alive
+#pragma unroll
+        for (int f = 0; f < 13; ++f) aA[0] += abl[f];
+        if (is_out && j == z1) D[gx + P.nx * gy + (long long)plane * (j - 1)] = aA[0] + ph_p;
+      } else if (is_out && j - 1 >= z0) {
         NodeOut<T> out;
         out.p = abl[0]; out.ux = abl[1]; out.uy = abl[2]; out.uz = abl[3];
         out.axx = abl[4]; out.ayy = abl[5]; out.azz = abl[6]; out.axy = abl[7];

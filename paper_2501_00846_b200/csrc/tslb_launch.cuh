@@ -95,6 +95,8 @@ bool tma_build_maps(const DevParams<T>& P, const T* S, const T* D, TmaMaps* m) {
     if (!tma_encode(&m->az[kind], dt, 3, S + 12 * P.N, sdims, sstr, sbox)) return false;
     if (!tma_encode(&m->ph[kind], dt, 3, D + F_PHI * P.N, sdims, sstr, sbox)) return false;
   }
+  const cuuint32_t fbox[4] = {cuuint32_t(M::W * Wel), cuuint32_t(M::HT), 1, 1};
+  if (!tma_encode(&m->vecf, dt, 4, S, vdims, vstr, fbox)) return false;
   return true;
 }
 
@@ -102,13 +104,14 @@ template <typename T> inline bool tma_usable(const DevParams<T>& P) {
   return P.nx % 32 == 0 && P.nx >= 64 && P.ny > 8;
 }
 
-template <typename T, int TY, int MINB, int NSTAGE, int ABL = 0, int PF = 0>
+template <typename T, int TY, int MINB, int NSTAGE, int ABL = 0, int PF = 0, bool SPLIT = false>
 cudaError_t launch_tma(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream, int zc,
                        TmaCache* tc) {
   constexpr int TX = 32;
   using M = TileMap<TX, TY, 1>;
-  auto kernel = k_stream_collide_tma<T, TX, TY, MINB, NSTAGE, ABL, PF>;
-  constexpr size_t smem = sizeof(K2FastSmem<T, M::CELLS, M::NMAIN>) + NSTAGE * sizeof(TmaStage<T, TX, TY>) +
+  auto kernel = k_stream_collide_tma<T, TX, TY, MINB, NSTAGE, ABL, PF, SPLIT>;
+  constexpr size_t smem = sizeof(K2FastSmem<T, M::CELLS, M::NMAIN>) +
+                          NSTAGE * sizeof(TmaStage<T, TX, TY, SPLIT>) +
                           NSTAGE * sizeof(unsigned long long);
   static_assert(smem <= 227 * 1024, "staging depth does not fit in shared memory");
   static bool ready = false;
@@ -278,7 +281,7 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
       e = walls ? launch_generic<T, true, NS>(P, S, D, stream) : launch_generic<T, false, NS>(P, S, D, stream);
   } else {
     int v2 = variant;
-    if (v2 >= 60 && v2 < 80 && !(tc && tma_usable(P))) v2 = 0;    // TMA staging needs full tile rows
+    if (v2 >= 57 && v2 < 80 && !(tc && tma_usable(P))) v2 = 0;    // TMA staging needs full tile rows
     switch (v2) {
       case 70: e = launch_ws<T, 2>(P, S, D, Q, stream, 64, tc); break;
       case 71: e = launch_ws<T, 2>(P, S, D, Q, stream, 32, tc); break;
@@ -293,6 +296,34 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
       case 66:   // + L2 prefetch one plane beyond the staging depth (0.817 against 0.829 ms in fp64)
         if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2, 0, 1>(P, S, D, Q, stream, 64, tc);
         else e = launch_tma<T, 8, 2, 2, 0, 1>(P, S, D, Q, stream, 64, tc);
+        break;
+      case 57:   // loads only, one box per field plane
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2, 3, 0, true>(P, S, D, Q, stream, 64, tc);
+        else e = launch_tma<T, 8, 2, 2, 3, 0, true>(P, S, D, Q, stream, 64, tc);
+        break;
+      case 58:   // loads only, fp32: one block per SM, four slots
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2, 3>(P, S, D, Q, stream, 64, tc);
+        else e = launch_tma<T, 8, 1, 4, 3>(P, S, D, Q, stream, 64, tc);
+        break;
+      case 59:   // production + one box per field plane
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2, 0, 0, true>(P, S, D, Q, stream, 64, tc);
+        else e = launch_tma<T, 8, 2, 2, 0, 0, true>(P, S, D, Q, stream, 64, tc);
+        break;
+      case 73:   // one box per field plane + L2 prefetch of the next plane
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2, 0, 1, true>(P, S, D, Q, stream, 64, tc);
+        else e = launch_tma<T, 8, 2, 2, 0, 1, true>(P, S, D, Q, stream, 64, tc);
+        break;
+      case 74:   // one box per field plane, 32 planes per block
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2, 0, 0, true>(P, S, D, Q, stream, 32, tc);
+        else e = launch_tma<T, 8, 2, 2, 0, 0, true>(P, S, D, Q, stream, 32, tc);
+        break;
+      case 63:   // timing ablation: loads only
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2, 3>(P, S, D, Q, stream, 64, tc);
+        else e = launch_tma<T, 8, 2, 2, 3>(P, S, D, Q, stream, 64, tc);
+        break;
+      case 64:   // timing ablation: stores only
+        if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2, 5>(P, S, D, Q, stream, 64, tc);
+        else e = launch_tma<T, 8, 2, 2, 5>(P, S, D, Q, stream, 64, tc);
         break;
       case 65:   // timing ablation: memory only (wrong results on purpose)
         if constexpr (sizeof(T) == 8) e = launch_tma<T, 8, 1, 2, 1>(P, S, D, Q, stream, 64, tc);
@@ -318,9 +349,10 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
         const long long tiles = (long long)((P.nx + 31) / 32) * ((P.ny + 7) / 8);
         const bool deep = tiles * ((P.nz + 63) / 64) >= 3LL * 148 * minb;
         if constexpr (sizeof(T) == 8) {
-          // fp64: TMA tensor staging two planes ahead where the tile rows are full (0.83 ms on
+          // fp64: TMA tensor staging two planes ahead where the tile rows are full (0.79 ms on
           // 256^3 against 0.85 ms with cp.async); it needs the depth, so only on deep grids
-          if (deep && tc && tma_usable(P)) e = launch_tma<T, 8, 1, 2>(P, S, D, Q, stream, 64, tc);
+          if (deep && tc && tma_usable(P))
+            e = launch_tma<T, 8, 1, 2, 0, 0, true>(P, S, D, Q, stream, 64, tc);   // one box per field plane
           else e = launch_fast<T, 8, 1, false, 0, 1>(P, S, D, Q, stream, deep ? 64 : 32);
         } else
           e = deep ? launch_fast<T, 8, 2, false, 0, 2>(P, S, D, Q, stream, 64)

@@ -159,7 +159,7 @@ def test_interface_row_kernel_variants(ref, k1v):
             assert not bad, (k1v, prec, n, bad)
 
 
-@pytest.mark.parametrize("nx,variant", [(96, 60), (96, 61), (64, 62), (128, 60), (96, 70), (64, 71), (128, 72)])
+@pytest.mark.parametrize("nx,variant", [(96, 60), (96, 61), (64, 62), (128, 60), (96, 70), (64, 71), (128, 72), (96, 59), (64, 73), (128, 74), (96, 66)])
 def test_tma_staged_kernel(ref, nx, variant):
     """Stream-collide kernel with TMA bulk staging (flags bits 8-15 = 60, 62; kept as a measured, rejected variant): x tiles that wrap
     on the left, on the right, on both sides (nx = 32) and not at all; ragged in y and z."""
