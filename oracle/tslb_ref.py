@@ -13,21 +13,30 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "tslb_ref.c")
 _LIB = os.path.join(_HERE, "libtslb_ref.so")
+# Conditioning twin (R22, section 9): the SAME source built with FMA contraction on, i.e.
+# another rounding at every multiply-add of every node and step.  Selected by the environment
+# variable TSLB_REF_FMA=1 before the first call; used only by tests/golden/make_golden.py
+# --twin-fma to measure how far two correct roundings of this oracle drift apart.  Expected
+# values always come from the contraction-off build.
+_LIB_FMA = os.path.join(_HERE, "libtslb_ref_fma.so")
 
 PERIODIC, WALL = 0, 1
 
 
-def build_lib(force=False):
-    """gcc -O3, contraction off (R22), OpenMP over nodes.  No -march flag: the .so travels."""
+def build_lib(force=False, fma=False):
+    """gcc -O3, contraction off (R22), OpenMP over nodes.  No -march flag: the .so travels.
+    fma=True builds the conditioning twin (contraction on, -mfma) next to it."""
     hdr = os.path.join(_HERE, "tslb_ref.h")
-    if (not force and os.path.exists(_LIB)
-            and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
-        return _LIB
-    tmp = _LIB + f".{os.getpid()}.tmp"       # build aside, then rename: a process that has the
-    subprocess.check_call(["gcc", "-O3", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+    out = _LIB_FMA if fma else _LIB
+    if (not force and os.path.exists(out)
+            and os.path.getmtime(out) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
+        return out
+    tmp = out + f".{os.getpid()}.tmp"        # build aside, then rename: a process that has the
+    flags = ["-ffp-contract=fast", "-mfma"] if fma else ["-ffp-contract=off"]
+    subprocess.check_call(["gcc", "-O3"] + flags + ["-fopenmp", "-fPIC", "-shared",
                            "-Wall", "-o", tmp, _SRC, "-lm"])       # old library mapped keeps it
-    os.replace(tmp, _LIB)
-    return _LIB
+    os.replace(tmp, out)
+    return out
 
 
 class Params(C.Structure):
@@ -54,7 +63,7 @@ _dp = C.POINTER(C.c_double)
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(build_lib())
+        _lib = C.CDLL(build_lib(fma=os.environ.get("TSLB_REF_FMA") == "1"))
         _lib.tslb_ref_create.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(Params),
                                          C.POINTER(C.c_void_p)]
         _lib.tslb_ref_init.argtypes = [C.c_void_p, _dp, _dp]

@@ -7,7 +7,12 @@ Usage:  python tests/golden/make_golden.py [--twin | --twin-only [--perturb-u]] 
         adds sens_<cp> from one perturbed ORACLE run, measured on the stored sample nodes;
         --perturb-u also perturbs the input velocity by 1e-21 (absolute, the size of the
         one-step rounding differences between two summation orders), which reaches the gas
-        phase where a relative perturbation of phi ~ 1e-9 is no perturbation at all)
+        phase where a relative perturbation of phi ~ 1e-9 is no perturbation at all;
+        --twin-fma [case ...]: instead of perturbing the input, run the SAME input through the
+        oracle source built with FMA contraction on (oracle/tslb_ref.py, TSLB_REF_FMA=1) and
+        store fma_<cp> = its distance from the stored expected values: two correct roundings of
+        one program, differing at every multiply-add of every step, which is what a CUDA kernel
+        with another summation order is too)
 
 For each case the oracle runs the seeded input of paper_2501_00846_b200.inputs for the
 config's full step count and stores, at the checkpoints {1, 10, 100, 1000, ..., final}:
@@ -36,11 +41,13 @@ import numpy as np
 ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 sys.path.insert(0, ROOT)
 
+if "--twin-fma" in sys.argv:
+    os.environ["TSLB_REF_FMA"] = "1"                   # before the oracle library is loaded
 from oracle import tslb_ref as R                      # noqa: E402
 from paper_2501_00846_b200 import inputs as I          # noqa: E402
 
 NSAMPLE = 2048
-HERE = os.path.dirname(os.path.abspath(__file__))
+HERE = os.environ.get("TSLB_GOLDEN_DIR", os.path.dirname(os.path.abspath(__file__)))
 
 
 def cases():
@@ -112,6 +119,32 @@ def run(name):
     np.savez_compressed(os.path.join(HERE, name + ".npz"), **out)
 
 
+def run_twin_fma(name):
+    """Add fma_<cp> to an existing golden file (the expected values are left untouched)."""
+    assert os.environ.get("TSLB_REF_FMA") == "1"
+    make, checkpoints = cases()[name]
+    path = os.path.join(HERE, name + ".npz")
+    cfg = make()
+    nz, ny, nx = cfg["shape"]
+    idx = np.load(path)["sample_index"]
+    twin = R.RefSim(nx, ny, nz, R.make_params(**cfg["params"]))
+    twin.init(cfg["phi"], cfg["u"])
+    done, t0 = 0, time.time()
+    for cp in checkpoints:
+        twin.step(cp - done)
+        done = cp
+        rho, p, u, phi = twin.get()
+        out = dict(np.load(path))                    # re-read: another twin may be writing too
+        got = (rho.ravel()[idx], p.ravel()[idx], u.reshape(3, -1)[:, idx], phi.ravel()[idx])
+        want = (out[f"rho_{cp}"], out[f"p_{cp}"], out[f"u_{cp}"], out[f"phi_{cp}"])
+        out[f"fma_{cp}"] = np.array([np.abs(a - b).max() / m
+                                     for a, b, m in zip(got, want, out[f"max_{cp}"])])
+        print(f"{name}: fma twin step {cp} after {time.time() - t0:.0f} s, drift = {out[f'fma_{cp}']}",
+              flush=True)
+        np.savez_compressed(path, **out)
+    twin.close()
+
+
 def run_twin_only(name):
     """Add sens_<cp> to an existing golden file: one perturbed oracle run against the stored
     sample values (the expected values themselves are left untouched)."""
@@ -147,7 +180,9 @@ def run_twin_only(name):
 if __name__ == "__main__":
     names = [a for a in sys.argv[1:] if not a.startswith("--")]
     for nm in (names or list(cases())):
-        if "--twin-only" in sys.argv:
+        if "--twin-fma" in sys.argv:
+            run_twin_fma(nm)
+        elif "--twin-only" in sys.argv:
             run_twin_only(nm)
         else:
             run(nm)
