@@ -165,6 +165,21 @@ cudaError_t launch_k1_flux(const DevParams<T>& P, const T* S, const T* Q, T* D, 
   return cudaGetLastError();
 }
 
+// Planes per block such that the grid fills whole waves of `slots` resident blocks: among the
+// chunk counts that give between 16 and 64 planes per block, the one with the best last wave.
+inline int balanced_zchunk(long long tiles_xy, int nz, int slots) {
+  int best = 32;
+  double best_eff = -1.0;
+  for (int nch = (nz + 63) / 64; nch <= (nz + 15) / 16; ++nch) {
+    const int zc = (nz + nch - 1) / nch;
+    const long long blocks = tiles_xy * ((nz + zc - 1) / zc);
+    const double waves = double(blocks) / slots;
+    const double eff = waves / double((long long)(waves + 0.999999)) * (double(zc) / (zc + 2));
+    if (eff > best_eff + 1e-9) { best_eff = eff; best = zc; }
+  }
+  return best;
+}
+
 // row kernel: V = 128 bit / sizeof(T) nodes per thread, zc planes per block
 template <typename T, int TY, int MINB, int NSTAGE>
 cudaError_t launch_k1_row(const DevParams<T>& P, const T* S, const T* Q, T* D, int zc,
@@ -243,11 +258,17 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
   int k1v = (flags >> 16) & 0xff;   // bits 16-23: tuning variant of the Allen-Cahn kernel
   const bool flux_form = !(P.bcx || P.bcy || P.bcz) && !(flags & 2) && (k1v == 0 || k1v >= 5);
   const bool row_ok = P.nx % RowVec<T>::V == 0;          // vector alignment of every row
-  if (flux_form && k1v == 0) k1v = row_ok ? 20 : 12;     // production choice, periodic
+  if (flux_form && k1v == 0) k1v = row_ok ? 35 : 12;     // production choice, periodic
   if (flux_form && k1v >= 20 && !row_ok) k1v = 12;
   switch (flux_form ? 100 + k1v : k1v) {
     case 112: e = launch_k1_flux<T, 8, 2, 3>(P, S, Q, D, stream); break;   // one node per thread
     case 120: e = launch_k1_row<T, 8, 2, 3>(P, S, Q, D, 32, stream); break;   // row kernel
+    case 135: {   // planes per block chosen for whole waves (2 blocks per SM, 148 SMs)
+      constexpr int V = RowVec<T>::V;
+      const long long txy = (long long)((P.nx + 32 * V - 1) / (32 * V)) * ((P.ny + 7) / 8);
+      e = launch_k1_row<T, 8, 2, 3>(P, S, Q, D, balanced_zchunk(txy, P.nz, 2 * 148), stream);
+      break;
+    }
     case 121: e = launch_k1_row<T, 8, 2, 3>(P, S, Q, D, 16, stream); break;
     case 122: e = launch_k1_row<T, 8, 2, 3>(P, S, Q, D, 64, stream); break;
     case 123: e = launch_k1_row<T, 8, 3, 2>(P, S, Q, D, 32, stream); break;

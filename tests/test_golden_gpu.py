@@ -5,6 +5,10 @@ in fp32), widened only where the TRAJECTORY ITSELF is ill-conditioned (DESIGN.md
 file records how far a second oracle run, perturbed by 1e-15 at t = 0, has drifted (sens); with
 A = sens/1e-15 the amplification, no arithmetic with unit round-off eps that rounds at every one
 of ~1000 steps can agree better than ~1000 eps A, so bar = max(tol, 1000 eps A).
+A perturbation at t = 0 under-estimates what rounding differently at EVERY step does, so the
+long case also records fma = the drift between the oracle and the SAME oracle source built with
+FMA contraction on (two correct fp64 roundings of one program, make_golden.py --twin-fma); a
+third rounding, the CUDA kernel, is allowed 10 x that (scaled by eps/eps64 in fp32).
 In fp32 the velocity of a STATIC droplet is a spurious current of 4e-5 and falling; there the
 relative bar is replaced by an absolute one of 1e-6 lattice units (Mach 2e-6), printed as such."""
 import os
