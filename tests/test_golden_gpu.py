@@ -69,17 +69,45 @@ def test_against_golden(case, precision):
         print(f"[{case} {precision}] step {cp}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items())
               + f" | sum(phi) rel diff {sum_phi / gold[f'diag_{cp}'][0] - 1:.1e}"
               + f" sum(p*) {sum_ps:.1e} (oracle {gold[f'diag_{cp}'][1]:.1e})")
-        sens = dict(zip(("rho", "p", "u", "phi"), gold[f"sens_{cp}"])) if f"sens_{cp}" in gold else {}
+        names = ("rho", "p", "u", "phi")
+        sens = dict(zip(names, gold[f"sens_{cp}"])) if f"sens_{cp}" in gold else {}
+        fma = dict(zip(names, gold[f"fma_{cp}"])) if f"fma_{cp}" in gold else {}
         eps = 1.1e-16 if precision == "f64" else 6e-8
+        # conditioning of the trajectory at this checkpoint, measured by the ORACLE alone: drift of
+        # a run perturbed by 1e-15 at t = 0 (sens) and of the same source built with FMA
+        # contraction, i.e. rounded differently at every step (fma).  Once two fp64 roundings of
+        # the oracle itself have drifted apart by more than a tenth of the tolerance, pointwise
+        # parity at that tolerance has no meaning any more (DESIGN.md 9 (3)).
+        cond = {k: max(float(sens.get(k, 0.0)), float(fma.get(k, 0.0))) for k in names}
+        ill = precision == "f64" and any(10.0 * cond[k] > 1e-10 for k in names)
         worst[cp] = {}
         for k in fields:
             bar = max(tol, 1000.0 * eps * float(sens.get(k, 0.0)) / 1e-15)
+            if ill:
+                bar = max(bar, 1e-3)          # "still the same flow"; the real checks are below
             ok = errs[k] <= bar
             if not ok and k == "u" and precision == "f32":
                 ok = errs[k] * float(gold[f"max_{cp}"][2]) <= 1e-6      # absolute, lattice units
             worst[cp][k] = (errs[k], bar, ok)
         if sens:
             print(f"    oracle sensitivity: " + " ".join(f"{k}={v:.1e}" for k, v in sens.items()))
+        if fma:
+            print(f"    oracle vs its FMA build: " + " ".join(f"{k}={v:.1e}" for k, v in fma.items()))
+        # what holds at any horizon: phi is conserved (P7), and the quantity BASELINE.json asks of
+        # the Laplace sweep at its final step, Delta p R_eff / (2 sigma) (pin P9's definition),
+        # agrees with the oracle's although the pointwise fields no longer can
+        if precision == "f64":
+            assert abs(sum_phi / gold[f"diag_{cp}"][0] - 1.0) <= 1e-12, (cp, sum_phi)
+            ratio_ref = float(gold[f"diag_{cp}"][2])
+            if np.isfinite(ratio_ref) and "droplet" in cfg["name"]:
+                phi_g, p_g = g["phi"].double(), g["p"].double()
+                dp = float(p_g[phi_g > 0.99].mean() - p_g[phi_g < 0.01].mean())
+                r_eff = (3.0 * sum_phi / (4.0 * np.pi)) ** (1.0 / 3.0)
+                ratio = dp * r_eff / (2.0 * cfg["params"]["sigma"])
+                print(f"    Laplace ratio {ratio:.9f} (oracle {ratio_ref:.9f})"
+                      + ("   [ill-conditioned checkpoint]" if ill else ""))
+                assert abs(ratio - ratio_ref) <= (1e-5 if ill else 1e-8) * max(1.0, abs(ratio_ref)), \
+                    (cp, ratio, ratio_ref)
         assert bool(torch.isfinite(g["u"]).all())
     s.close()
     bad = {cp: e for cp, e in worst.items() if any(not ok for _, _, ok in e.values())}
