@@ -65,8 +65,10 @@ typedef struct tslb_params {
 size_t tslb_workspace_bytes(int nx, int ny, int nz, const tslb_params *params);
 
 /* Create a solver on the CALLER-OWNED device buffer `workspace` (>= tslb_workspace_bytes,
- * 256-byte aligned, kept alive until tslb_destroy).  The library carves its double-buffered SoA
- * planes out of it and allocates nothing else on the device.  `stream` is a cudaStream_t (NULL =
+ * 256-byte aligned, kept alive until tslb_destroy).  The library carves out of it two state
+ * buffers of 14 SoA planes, 3 more planes for the Allen-Cahn flux Q that the two kernels of a step
+ * hand to each other (31 planes while the step is a split pair), and the partial-sum
+ * rows of tslb_diag; it allocates nothing else on the device.  `stream` is a cudaStream_t (NULL =
  * legacy default stream).  Minimum size: 4 nodes on a periodic axis, 2 on a wall axis.  No
  * kernel is launched. */
 int tslb_create(int nx, int ny, int nz, const tslb_params *params, void *workspace, void *stream,
@@ -88,6 +90,28 @@ int tslb_get(tslb_handle *h, void *rho, void *p, void *u, void *phi);
 /* Full internal state (debug / parity of the unexposed fields): p*[N], u[3][N], a2_neq[6][N] in
  * the order xx,yy,zz,xy,xz,yz, a[3][N], phi[N]; DEVICE arrays, NULL skips. */
 int tslb_get_state(tslb_handle *h, void *pstar, void *u, void *A, void *a, void *phi);
+
+/* On-device diagnostics: box reductions of the current state, the
+ * quantities behind the paper's validation plots (centre-of-mass velocity of a rising bubble,
+ * Fig. 4) and BASELINE.json's checks (sum(phi) conserved; Laplace's law
+ * Delta p R/(2 sigma) on configs[1]), so that no whole field has to be read back.
+ * out = TSLB_NDIAG doubles (fp64 accumulation in both precisions), indexed by TSLB_D_*:
+ *   SUM_PHI, SUM_PSTAR, MAX_U (max |u|), SUM_PHI_X/Y/Z (sum phi * node index: centre of mass of
+ *   the liquid = SUM_PHI_X / SUM_PHI on a non-periodic axis), SUM_PHI_UX/UY/UZ (its momentum per
+ *   unit liquid density), SUM_UX/UY/UZ (so the light phase's is sum(u) - sum(phi u)),
+ *   SUM_P_IN / N_IN: sum and count of p = p* rho cs^2 over nodes with phi > 0.99,
+ *   SUM_P_OUT / N_OUT: the same over phi < 0.01 (Delta p = SUM_P_IN/N_IN - SUM_P_OUT/N_OUT).
+ * Two launches on the handle's stream, deterministic (fixed reduction order, no atomics); the
+ * partial sums live in the caller's workspace.  tslb_diag writes a DEVICE array and does not
+ * synchronise; tslb_diag_host writes a HOST array and synchronises the stream. */
+enum { TSLB_D_SUM_PHI = 0, TSLB_D_SUM_PSTAR = 1, TSLB_D_MAX_U = 2,
+       TSLB_D_SUM_PHI_X = 3, TSLB_D_SUM_PHI_Y = 4, TSLB_D_SUM_PHI_Z = 5,
+       TSLB_D_SUM_PHI_UX = 6, TSLB_D_SUM_PHI_UY = 7, TSLB_D_SUM_PHI_UZ = 8,
+       TSLB_D_SUM_UX = 9, TSLB_D_SUM_UY = 10, TSLB_D_SUM_UZ = 11,
+       TSLB_D_SUM_P_IN = 12, TSLB_D_N_IN = 13, TSLB_D_SUM_P_OUT = 14, TSLB_D_N_OUT = 15,
+       TSLB_NDIAG = 16 };
+int tslb_diag(tslb_handle *h, double *out);
+int tslb_diag_host(tslb_handle *h, double *out);
 
 /* Host-buffer convenience for end-to-end use: same as tslb_init / tslb_get but the field
  * pointers are HOST arrays (pinned memory makes the copies asynchronous); the library stages

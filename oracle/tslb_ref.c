@@ -483,3 +483,55 @@ int tslb_ref_get_state(tslb_ref *h, double *pstar, double *u, double *A, double 
   if (phi) memcpy(phi, h->phi, N * sizeof(double));
   return 0;
 }
+
+/* Restart aid for the segment-parity tests: replace the whole state by the
+ * caller's arrays.  Copies only, no arithmetic; afterwards tslb_ref_step continues from it. */
+int tslb_ref_set_state(tslb_ref *h, const double *pstar, const double *u, const double *A,
+                       const double *a, const double *phi) {
+  if (!h || !pstar || !u || !A || !a || !phi) return -1;
+  long N = h->N;
+  memcpy(h->pstar, pstar, N * sizeof(double));
+  memcpy(h->u, u, 3 * N * sizeof(double));
+  memcpy(h->A, A, 6 * N * sizeof(double));
+  memcpy(h->a, a, 3 * N * sizeof(double));
+  memcpy(h->phi, phi, N * sizeof(double));
+  h->inited = 1;
+  return 0;
+}
+
+/* Diagnostics of the current state: the box reductions behind what the
+ * paper plots (centre-of-mass velocity of a bubble, Fig. 4) and what
+ * BASELINE.json checks (conservation of sum(phi), Laplace's law).  Plain loops in node order,
+ * long double accumulators.  out[16]:
+ *    0 sum(phi)   1 sum(p*)   2 max |u|
+ *    3..5  sum(phi ix), sum(phi iy), sum(phi iz)          (node indices as coordinates)
+ *    6..8  sum(phi u)        9..11 sum(u)
+ *   12 sum of p over nodes with phi > 0.99, 13 their count           (p = p* rho cs^2)
+ *   14 sum of p over nodes with phi < 0.01, 15 their count */
+int tslb_ref_diag(tslb_ref *h, double out[16]) {
+  if (!h || !out) return -1;
+  if (!h->inited) return -4;
+  long N = h->N;
+  long double s[16];
+  for (int k = 0; k < 16; ++k) s[k] = 0.0L;
+  double umax = 0.0;
+  for (int iz = 0; iz < h->nz; ++iz)
+    for (int iy = 0; iy < h->ny; ++iy)
+      for (int ix = 0; ix < h->nx; ++ix) {
+        long x = ix + (long)h->nx * (iy + (long)h->ny * iz);
+        double ph = h->phi[x];
+        double ux = h->u[x], uy = h->u[N + x], uz = h->u[2 * N + x];
+        double p = h->pstar[x] * mix_rho(&h->p, ph) * CS2;
+        double um = sqrt(ux * ux + uy * uy + uz * uz);
+        if (um > umax) umax = um;
+        s[0] += ph; s[1] += h->pstar[x];
+        s[3] += ph * ix; s[4] += ph * iy; s[5] += ph * iz;
+        s[6] += ph * ux; s[7] += ph * uy; s[8] += ph * uz;
+        s[9] += ux; s[10] += uy; s[11] += uz;
+        if (ph > 0.99) { s[12] += p; s[13] += 1.0L; }
+        if (ph < 0.01) { s[14] += p; s[15] += 1.0L; }
+      }
+  for (int k = 0; k < 16; ++k) out[k] = (double)s[k];
+  out[2] = umax;
+  return 0;
+}

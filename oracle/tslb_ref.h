@@ -51,6 +51,13 @@ int  tslb_ref_step   (tslb_ref *h, int n);
 int  tslb_ref_get    (tslb_ref *h, double *rho, double *p, double *u, double *phi); /* NULL = skip */
 int  tslb_ref_get_state(tslb_ref *h, double *pstar, double *u, double *A, double *a, double *phi);
 void tslb_ref_destroy(tslb_ref *h);
+/* Restart aid for segment parity (copies only): replace the whole state; A is a2_neq itself. */
+int  tslb_ref_set_state(tslb_ref *h, const double *pstar, const double *u, const double *A,
+                        const double *a, const double *phi);
+/* Box reductions of the current state (Fig. 4, 292):
+ * out[16] = sum(phi), sum(p*), max|u|, sum(phi ix,iy,iz), sum(phi u), sum(u),
+ * sum and count of p = p* rho cs^2 over phi > 0.99, the same over phi < 0.01. */
+int  tslb_ref_diag(tslb_ref *h, double out[16]);
 
 /* Single-node pieces, the same functions the passes call, exported so the pins can reach them. */
 void tslb_ref_lattice(int c[27][3], double w[27], int opp[27]);          /* R1            */

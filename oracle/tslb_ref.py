@@ -70,6 +70,8 @@ def lib():
         _lib.tslb_ref_step.argtypes = [C.c_void_p, C.c_int]
         _lib.tslb_ref_get.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
         _lib.tslb_ref_get_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
+        _lib.tslb_ref_set_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
+        _lib.tslb_ref_diag.argtypes = [C.c_void_p, _dp]
         _lib.tslb_ref_destroy.argtypes = [C.c_void_p]
         _lib.tslb_ref_destroy.restype = None
         _lib.tslb_ref_omega.argtypes = [C.POINTER(Params), C.c_double]
@@ -126,6 +128,21 @@ class RefSim:
         rc = lib().tslb_ref_get_state(self._h, _p(ps), _p(u), _p(A), _p(a), _p(phi))
         assert rc == 0, rc
         return ps, u, A, a, phi
+
+    def set_state(self, pstar, u, A, a, phi):
+        """Replace the whole state (a2_neq itself in A); copies only (segment-parity restarts)."""
+        arrs = [_f64(x) for x in (pstar, u, A, a, phi)]
+        want = [self.shape, (3,) + self.shape, (6,) + self.shape, (3,) + self.shape, self.shape]
+        assert [x.shape for x in arrs] == want
+        rc = lib().tslb_ref_set_state(self._h, *[_p(x) for x in arrs])
+        assert rc == 0, rc
+
+    def diag(self):
+        """tslb_ref_diag: the 16 box reductions, in the order of include/tslb.h's TSLB_D_*."""
+        out = np.empty(16)
+        rc = lib().tslb_ref_diag(self._h, _p(out))
+        assert rc == 0, rc
+        return out
 
     def close(self):
         if self._h:

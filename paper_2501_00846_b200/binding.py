@@ -14,10 +14,14 @@ LIB_PATH = os.path.join(_HERE, "libtslb.so")
 BC_PERIODIC, BC_WALL = 0, 1
 F32, F64 = 0, 1
 FLAG_NAIVE = 1
+NDIAG = 16
+DIAG_NAMES = ("sum_phi", "sum_pstar", "max_u", "sum_phi_x", "sum_phi_y", "sum_phi_z",
+              "sum_phi_ux", "sum_phi_uy", "sum_phi_uz", "sum_ux", "sum_uy", "sum_uz",
+              "sum_p_in", "n_in", "sum_p_out", "n_out")
 
 SYMBOLS = ("tslb_workspace_bytes", "tslb_create", "tslb_init", "tslb_step", "tslb_get",
            "tslb_get_state", "tslb_init_host", "tslb_get_host", "tslb_step_timed",
-           "tslb_launch_count",
+           "tslb_launch_count", "tslb_diag", "tslb_diag_host",
            "tslb_destroy", "tslb_last_error")
 
 
@@ -64,6 +68,8 @@ def load():
     lib.tslb_init_host.argtypes = [vp, vp, vp]
     lib.tslb_get_host.argtypes = [vp, vp, vp, vp, vp]
     lib.tslb_step_timed.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
+    lib.tslb_diag.argtypes = [vp, vp]
+    lib.tslb_diag_host.argtypes = [vp, C.POINTER(C.c_double)]
     lib.tslb_launch_count.argtypes = [vp]
     lib.tslb_launch_count.restype = C.c_longlong
     lib.tslb_destroy.argtypes = [vp]
@@ -166,6 +172,18 @@ class Solver:
         _check(self.lib.tslb_get_state(self._h, out["pstar"].data_ptr(), out["u"].data_ptr(),
                                        out["A"].data_ptr(), out["a"].data_ptr(),
                                        out["phi"].data_ptr()), "tslb_get_state")
+        return out
+
+    def diag(self):
+        """tslb_diag_host: dict of the TSLB_D_* box reductions (synchronises the stream)."""
+        out = (C.c_double * NDIAG)()
+        _check(self.lib.tslb_diag_host(self._h, out), "tslb_diag_host")
+        return dict(zip(DIAG_NAMES, out))
+
+    def diag_device(self):
+        """tslb_diag into a device tensor of NDIAG doubles (no synchronisation)."""
+        out = self.torch.empty(NDIAG, dtype=self.torch.float64, device=self.device)
+        _check(self.lib.tslb_diag(self._h, out.data_ptr()), "tslb_diag")
         return out
 
     def get_host(self, out):

@@ -13,6 +13,7 @@
 #include "tslb_device.cuh"
 #include "tslb_naive.cuh"
 #include "tslb_launch.cuh"
+#include "tslb_diag.cuh"
 
 namespace {
 
@@ -52,6 +53,9 @@ size_t elem_size(const tslb_params* p) { return p->precision == TSLB_F64 ? 8 : 4
 // bytes of one SoA plane, padded so that every plane starts 256-byte aligned
 size_t plane_bytes(long long N, size_t es) { return round_up(size_t(N) * es); }
 int scratch_planes(const tslb_params*) { return 3; }   // Allen-Cahn flux Q (or naive scratch)
+// diagnostics region at the end of the workspace: one row of NDIAG doubles per DIAG_NODES nodes
+// (partial sums of tslb_diag) and one more row for the result of tslb_diag_host
+size_t diag_bytes(long long N) { return round_up(size_t(tslb::diag_rows(N) + 1) * tslb::NDIAG * 8); }
 
 template <typename T>
 tslb::DevParams<T> make_dev(int nx, int ny, int nz, const tslb_params& p, long long stride) {
@@ -80,6 +84,7 @@ struct tslb_handle {
   cudaStream_t stream;
   char* buf[2];          // two state buffers of NFIELD planes
   char* scratch;         // 3 planes: flux Q of Eq. 20 (periodic path) / naive-path scratch
+  double* diag;          // diag_rows(nodes) + 1 rows of NDIAG doubles (tslb_diag partial sums)
   int cur;
   bool inited;
   long long launches;
@@ -93,7 +98,7 @@ const char* tslb_last_error(void) { return g_err; }
 size_t tslb_workspace_bytes(int nx, int ny, int nz, const tslb_params* p) {
   if (!params_ok(nx, ny, nz, p)) return 0;
   size_t pb = plane_bytes((long long)nx * ny * nz, elem_size(p));
-  return pb * size_t(2 * tslb::NFIELD + scratch_planes(p));
+  return pb * size_t(2 * tslb::NFIELD + scratch_planes(p)) + diag_bytes((long long)nx * ny * nz);
 }
 
 int tslb_create(int nx, int ny, int nz, const tslb_params* p, void* workspace, void* stream,
@@ -116,6 +121,7 @@ int tslb_create(int nx, int ny, int nz, const tslb_params* p, void* workspace, v
   h->buf[0] = w;
   h->buf[1] = w + pb * tslb::NFIELD;
   h->scratch = scratch_planes(p) ? w + pb * 2 * tslb::NFIELD : nullptr;
+  h->diag = reinterpret_cast<double*>(w + pb * size_t(2 * tslb::NFIELD + scratch_planes(p)));
   h->cur = 0;
   h->inited = false;
   h->launches = 0;
@@ -252,6 +258,42 @@ int tslb_get_state(tslb_handle* h, void* pstar, void* u, void* A, void* a, void*
   }
   h->launches += 1;
   CUDA_TRY(cudaGetLastError());
+  return TSLB_OK;
+}
+
+// partial sums into `rows` (device scratch of diag_rows(nodes) rows), result into `out` (device)
+static int diag_launch(tslb_handle* h, double* rows, double* out) {
+  const unsigned blocks = unsigned(tslb::diag_rows(h->nodes));
+  if (h->prm.precision == TSLB_F64) {
+    auto P = make_dev<double>(h->nx, h->ny, h->nz, h->prm, h->stride);
+    tslb::k_diag_partial<double><<<blocks, tslb::DIAG_THREADS, 0, h->stream>>>(
+        P, h->nodes, reinterpret_cast<const double*>(h->buf[h->cur]), rows);
+  } else {
+    auto P = make_dev<float>(h->nx, h->ny, h->nz, h->prm, h->stride);
+    tslb::k_diag_partial<float><<<blocks, tslb::DIAG_THREADS, 0, h->stream>>>(
+        P, h->nodes, reinterpret_cast<const float*>(h->buf[h->cur]), rows);
+  }
+  tslb::k_diag_final<<<1, tslb::DIAG_THREADS, 0, h->stream>>>(rows, (long long)blocks, out);
+  h->launches += 2;
+  CUDA_TRY(cudaGetLastError());
+  return TSLB_OK;
+}
+
+int tslb_diag(tslb_handle* h, double* out) {
+  if (!h || !out) return fail(TSLB_EINVAL, "tslb_diag: NULL argument");
+  if (!h->inited) return fail(TSLB_ESTATE, "tslb_diag before tslb_init");
+  return diag_launch(h, h->diag, out);
+}
+
+int tslb_diag_host(tslb_handle* h, double* out) {
+  if (!h || !out) return fail(TSLB_EINVAL, "tslb_diag_host: NULL argument");
+  if (!h->inited) return fail(TSLB_ESTATE, "tslb_diag_host before tslb_init");
+  double* d_out = h->diag + tslb::diag_rows(h->nodes) * tslb::NDIAG;
+  int rc = diag_launch(h, h->diag, d_out);
+  if (rc != TSLB_OK) return rc;
+  CUDA_TRY(cudaMemcpyAsync(out, d_out, tslb::NDIAG * sizeof(double), cudaMemcpyDeviceToHost,
+                           h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
   return TSLB_OK;
 }
 

@@ -196,6 +196,33 @@ def head_on_collision(n=256, radius=24.0, half_sep=40.0, speed=0.05, seed=3, noi
     return dict(name=f"head_on_collision_{n}", shape=shape, params=prm, phi=phi1 + phi2, u=u)
 
 
+def off_axis_collision(n=256, impact=0.38, weber=53.0, radius=None, half_sep=None, speed=0.05,
+                       seed=4, noise=1e-6):
+    """off-axis binary collision.  As head_on_collision, but
+    the droplet centres are offset by b = impact * D along y, perpendicular to the relative
+    velocity (`impact` = the paper's x, "the ratio of the distance between the centers of the
+    droplets and their diameter", 0.28-0.5 there).  Oh = sqrt(We)/Re is kept at the paper's
+    0.0044, so Re follows from We (We 53 -> Re 1655).  rho ratio 800, mu ratio 50 as configs[3].
+    Sizes scale with the box like bench.py's collision workload (R = 24, half_sep = 40 at 256)."""
+    shape = (n, n, n)
+    s = n / 256.0
+    radius = 24.0 * s if radius is None else radius
+    half_sep = 40.0 * s if half_sep is None else half_sep
+    U, D = 2.0 * speed, 2.0 * radius
+    sigma = 1.0 * U * U * D / weber
+    reynolds = np.sqrt(weber) / 0.0044
+    mu_l = U * D / reynolds
+    prm = base_params(rho_g=1.0 / 800.0, sigma=sigma, mu_l=mu_l, mu_g=mu_l / 50.0)
+    c = (n - 1) / 2.0
+    b = 0.5 * impact * D
+    phi1 = sphere_profile(shape, (c - half_sep, c - b, c), radius, prm["delta"], prm["bc"])
+    phi2 = sphere_profile(shape, (c + half_sep, c + b, c), radius, prm["delta"], prm["bc"])
+    u = noise_u(shape, noise, seed) if noise else np.zeros((3,) + shape)
+    u[0] += speed * phi1 - speed * phi2
+    return dict(name=f"off_axis_collision_{n}_x{impact:g}_We{weber:g}", shape=shape, params=prm,
+                phi=phi1 + phi2, u=u)
+
+
 def emulsion_sweep(n=384, n_drops=200, seed=5):
     """configs[4]: 200 droplets, radii in [6,14], solenoidal velocity of amplitude 0.02."""
     shape = (n, n, n)
