@@ -113,6 +113,21 @@ enum { TSLB_D_SUM_PHI = 0, TSLB_D_SUM_PSTAR = 1, TSLB_D_MAX_U = 2,
 int tslb_diag(tslb_handle *h, double *out);
 int tslb_diag_host(tslb_handle *h, double *out);
 
+/* Allocation-free variant of tslb_diag, for callers that cannot provide or allocate scratch
+ * (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): same kernels, same
+ * result bit for bit, but the partial sums live in a static device array inside the library
+ * (512 KB, held by every GPU that loads the library until the process exits) instead of the
+ * workspace.  The call allocates nothing and synchronises nothing; `out` is a DEVICE array of
+ * TSLB_NDIAG doubles; the handle's device must be the current device.
+ * Limit: lattices of at most TSLB_DIAG_STATIC_MAX_NODES nodes (256^3 and 320^3 fit, 384^3 does
+ * not); larger ones return TSLB_EINVAL with a text that says so (use tslb_diag).
+ * The array is shared by every handle and every call in the process and keeps the last call's
+ * contents (no call depends on them: every row read is overwritten first): calls whose kernels
+ * may overlap on the GPU (different streams, no ordering between them) RACE on it; calls on one
+ * stream, or ordered by events, are safe. */
+enum { TSLB_DIAG_STATIC_MAX_NODES = 4096 * 8192 };
+int tslb_diag_static(tslb_handle *h, double *out);
+
 /* Host-buffer convenience for end-to-end use: same as tslb_init / tslb_get but the field
  * pointers are HOST arrays (pinned memory makes the copies asynchronous); the library stages
  * them through the spare state buffer, so no extra device memory is needed.  tslb_get_host

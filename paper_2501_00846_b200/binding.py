@@ -21,7 +21,7 @@ DIAG_NAMES = ("sum_phi", "sum_pstar", "max_u", "sum_phi_x", "sum_phi_y", "sum_ph
 
 SYMBOLS = ("tslb_workspace_bytes", "tslb_create", "tslb_init", "tslb_step", "tslb_get",
            "tslb_get_state", "tslb_init_host", "tslb_get_host", "tslb_step_timed",
-           "tslb_launch_count", "tslb_diag", "tslb_diag_host",
+           "tslb_launch_count", "tslb_diag", "tslb_diag_host", "tslb_diag_static",
            "tslb_destroy", "tslb_last_error")
 
 
@@ -70,6 +70,7 @@ def load():
     lib.tslb_step_timed.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
     lib.tslb_diag.argtypes = [vp, vp]
     lib.tslb_diag_host.argtypes = [vp, C.POINTER(C.c_double)]
+    lib.tslb_diag_static.argtypes = [vp, vp]
     lib.tslb_launch_count.argtypes = [vp]
     lib.tslb_launch_count.restype = C.c_longlong
     lib.tslb_destroy.argtypes = [vp]
@@ -184,6 +185,17 @@ class Solver:
         """tslb_diag into a device tensor of NDIAG doubles (no synchronisation)."""
         out = self.torch.empty(NDIAG, dtype=self.torch.float64, device=self.device)
         _check(self.lib.tslb_diag(self._h, out.data_ptr()), "tslb_diag")
+        return out
+
+    def diag_static(self, out=None):
+        """tslb_diag_static (no workspace scratch, no allocation inside the library) into the
+        caller's device tensor `out` of NDIAG doubles (made here if None); no synchronisation."""
+        if out is None:
+            out = self.torch.empty(NDIAG, dtype=self.torch.float64, device=self.device)
+        assert out.dtype == self.torch.float64 and out.numel() == NDIAG and out.is_contiguous()
+        assert out.device == self.device
+        with self.torch.cuda.device(self.device):
+            _check(self.lib.tslb_diag_static(self._h, out.data_ptr()), "tslb_diag_static")
         return out
 
     def get_host(self, out):

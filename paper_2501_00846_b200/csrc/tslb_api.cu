@@ -297,6 +297,56 @@ int tslb_diag_host(tslb_handle* h, double* out) {
   return TSLB_OK;
 }
 
+// ---- tslb_diag_static: the allocation-free variant ------------------------------------------
+// Same two kernels as tslb_diag, but the partial-sum rows live in a file-scope device array
+// instead of the caller's workspace, for callers that cannot hand over (or allocate) scratch:
+// code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Every GPU
+// that loads the library holds the array (512 KB) until the process exits.
+constexpr long long kDiagStaticRows = TSLB_DIAG_STATIC_MAX_NODES / tslb::DIAG_NODES;
+static_assert(kDiagStaticRows * tslb::DIAG_NODES == TSLB_DIAG_STATIC_MAX_NODES, "whole rows");
+static __device__ __align__(256) double g_diag_static_rows[kDiagStaticRows * tslb::NDIAG];
+
+// In host code the name g_diag_static_rows is a host-side stand-in, not a device address: its
+// device address is looked up with cudaGetSymbolAddress, once per device, with that device
+// current (device code could name the array directly; only the host needs the address).
+static int diag_static_rows(double** rows) {
+  constexpr int kMaxDev = 64;
+  static double* ptr[kMaxDev] = {};
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDev) return fail(TSLB_ECUDA, "tslb_diag_static: device ordinal out of range");
+  if (!ptr[dev]) {
+    void* p = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress(&p, g_diag_static_rows));
+    ptr[dev] = static_cast<double*>(p);
+  }
+  *rows = ptr[dev];
+  return TSLB_OK;
+}
+
+int tslb_diag_static(tslb_handle* h, double* out) {
+  if (!h || !out) return fail(TSLB_EINVAL, "tslb_diag_static: NULL argument");
+  if (h->nodes > (long long)TSLB_DIAG_STATIC_MAX_NODES) {
+    snprintf(g_err, sizeof(g_err),
+             "tslb_diag_static: lattice of %lld nodes exceeds the static scratch (at most %lld "
+             "nodes); use tslb_diag", h->nodes, (long long)TSLB_DIAG_STATIC_MAX_NODES);
+    return TSLB_EINVAL;
+  }
+  if (!h->inited) return fail(TSLB_ESTATE, "tslb_diag_static before tslb_init");
+  // the array belongs to the CURRENT device: it must be the one the handle's workspace is on
+  cudaPointerAttributes at;
+  int dev = -1;
+  CUDA_TRY(cudaPointerGetAttributes(&at, h->buf[0]));
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (at.type == cudaMemoryTypeDevice && at.device != dev)
+    return fail(TSLB_EINVAL, "tslb_diag_static: the handle's device is not the current device");
+  double* rows = nullptr;
+  int rc = diag_static_rows(&rows);
+  if (rc != TSLB_OK) return rc;
+  // nothing has to start at zero: k_diag_partial overwrites every row k_diag_final reads
+  return diag_launch(h, rows, out);
+}
+
 int tslb_init_host(tslb_handle* h, const void* phi, const void* u) {
   if (!h || !phi || !u) return fail(TSLB_EINVAL, "tslb_init_host: NULL argument");
   // stage phi, u in planes 0..3 of the second buffer, then run the init kernel into buffer 0
