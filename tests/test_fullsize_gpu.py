@@ -101,3 +101,51 @@ def test_mirror_symmetry_and_translation_at_full_size():
     assert float((b["phi"] - torch.roll(phi, sh, (0, 1, 2))).abs().max()) < 1e-10
     assert float((b["u"] - torch.roll(u, sh, (1, 2, 3))).abs().max()) < 1e-10 * float(u.abs().max())
     s.close()
+
+
+# ---------------------------------------------------------------- whole field at 256^3 ----
+FULL_STEPS = 3
+
+
+@pytest.fixture(scope="module")
+def oracle_full(ref, workload):
+    """The oracle on the WHOLE 256^3 input for a few steps (~12 GB of host memory, a few
+    seconds per step on the GPU box's cores): every node of the production launch configuration
+    is compared, so the 64-plane chunk seams, the wrapped column / row / corner boxes of the TMA
+    staging and the slot parity over many planes are all covered element by element."""
+    cfg = workload
+    sim = ref.RefSim(N, N, N, ref.make_params(**cfg["params"]))
+    sim.init(cfg["phi"], cfg["u"])
+    sim.step(FULL_STEPS)
+    out = dict(zip(("rho", "p", "u", "phi"), sim.get()))
+    out["pstar"], _, _, out["a"], _ = sim.get_state()
+    sim.close()
+    return out
+
+
+@pytest.mark.parametrize("precision,tol", [("f64", 1e-10), ("f32", 1e-4)])
+def test_whole_field_against_oracle(oracle_full, workload, precision, tol):
+    """flags = 0: the kernels bench.py times (fp64: TMA-staged stream-collide, fp32: cp.async
+    two planes ahead, 64-plane chunks; row kernel for the interface), full field, element by
+    element, after FULL_STEPS steps."""
+    import torch
+    from paper_2501_00846_b200 import binding as B
+    cfg, want = workload, oracle_full
+    s = B.Solver(N, N, N, cfg["params"], precision=precision)
+    s.init(cfg["phi"], cfg["u"])
+    s.step(FULL_STEPS)
+    g = s.get()
+    st = s.get_state()
+    got = {k: v for k, v in g.items()} | {"pstar": st["pstar"], "a": st["a"]}
+    errs = {}
+    for k, w in want.items():
+        wt = torch.from_numpy(w).to("cuda")
+        errs[k] = float((got[k].double() - wt).abs().max() / wt.abs().max())
+        del wt
+    s.close()
+    print(f"[256^3 whole field, {precision}, {FULL_STEPS} steps] "
+          + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+    fields = ("rho", "p", "u", "phi") if precision == "f64" else ("u", "phi")
+    assert all(errs[k] <= tol for k in fields), errs
+    if precision == "f64":
+        assert errs["pstar"] <= 1e-9 and errs["a"] <= 1e-9, errs

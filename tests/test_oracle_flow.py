@@ -223,3 +223,45 @@ def test_p15_poiseuille(ref):
     z = np.arange(nz)
     exact = a / (2 * nu) * (z + 0.5) * (nz - 0.5 - z)
     assert np.abs(ux - exact).max() / np.abs(exact).max() < 2e-3
+
+
+# ---------------------------------------------------------------- P16 ------------------
+def _mirror_extend(a, axes, odd):
+    """Even (odd=False) or all-component odd (odd=True) mirror extension of a (..., nz, ny, nx)
+    array across walls half a cell outside the first/last node of the given array axes: the
+    periodic box of twice the length that a walled box stands for."""
+    for ax in axes:
+        m = np.flip(a, axis=ax)
+        a = np.concatenate([a, -m if odd else m], axis=ax)
+    return a
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 1), (1, 1, 0), (1, 1, 1)])
+def test_p16_allen_cahn_wall_ghosts_are_the_mirrored_box(ref, bc):
+    """Which ghost rule Eq. 20's two fluxes use at a wall (R19; P:292, P:358 neutral wetting):
+    one oracle step of phi on a walled box, droplet touching the walls, must equal the same step
+    on the periodic box of twice the length in which phi is mirrored evenly and u oddly (every
+    component: no slip).  In that box the sharpening flux phi(1-phi)n, built from mirrored
+    scalars, has an odd wall-normal and EVEN tangential components (ghost rule 1), the advective
+    flux phi u is odd in every component (rule 0).  Swapping either rule in pass_allen_cahn
+    changes phi^{n+1} next to the wall by ~1e-3 here (checked by mutation)."""
+    shape = (10, 9, 8)                                       # (nz, ny, nx)
+    prm = I.base_params(bc=bc)
+    phi = I.sphere_profile(shape, (1.3, 2.1, 1.6), 3.5, 4.0, bc)     # touches the low walls
+    u = I.noise_u(shape, 2e-2, 41)
+    sim = ref.RefSim(shape[2], shape[1], shape[0], ref.make_params(**prm))
+    sim.init(phi, u)
+    sim.step(1)
+    got = sim.get()[3]
+    sim.close()
+    axes = [2 - d for d in range(3) if bc[d]]                # array axis of lattice axis d
+    phi2 = _mirror_extend(phi, axes, odd=False)
+    u2 = _mirror_extend(u, [1 + a for a in axes], odd=True)
+    big = ref.RefSim(phi2.shape[2], phi2.shape[1], phi2.shape[0],
+                     ref.make_params(**I.base_params()))
+    big.init(phi2, u2)
+    big.step(1)
+    want = big.get()[3][:shape[0], :shape[1], :shape[2]]
+    big.close()
+    assert np.abs(got - phi).max() > 1e-4                    # the step did something
+    assert np.abs(got - want).max() < 1e-14, np.abs(got - want).max()
