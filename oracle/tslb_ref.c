@@ -10,6 +10,15 @@
 #include <string.h>
 
 #define Q 27
+/* Order of the sums over the 27 directions (stencils, Eq. 18-19; moments, Eq. 11-13).  The paper
+ * does not fix it (R22).  The oracle sums in index order; -DTSLB_REF_REVERSE_SUMS builds the
+ * conditioning twin that sums in reverse order (make_golden.py --twin-rev): another correct
+ * rounding of the same program, never a source of expected values. */
+#ifdef TSLB_REF_REVERSE_SUMS
+#define FOR_SUM_Q(i) for (int i = Q - 1; i >= 0; --i)
+#else
+#define FOR_SUM_Q(i) for (int i = 0; i < Q; ++i)
+#endif
 #define OMP_MIN_NODES 8192   /* below this a pass runs on one thread (team start-up costs more) */
 static const double CS2 = 1.0 / 3.0;     /* R1: cs^2 of D3Q27                       */
 static const double EPS_N = 1e-12;       /* R13: n = grad(phi)/sqrt(|grad(phi)|^2 + eps^2) */
@@ -160,7 +169,7 @@ static double ghost_sign(const nbr_t *nb, int al, int rule) {
 static void grad_at(const double *psi, int ix, int iy, int iz, int nx, int ny, int nz,
                     const int bc[3], double g[3]) {
   g[0] = g[1] = g[2] = 0.0;
-  for (int i = 0; i < Q; ++i) {
+  FOR_SUM_Q(i) {
     nbr_t nb = neighbour(ix + Ci[i][0], iy + Ci[i][1], iz + Ci[i][2], nx, ny, nz, bc);
     for (int al = 0; al < 3; ++al) g[al] += Wi[i] * psi[nb.idx] * Ci[i][al];
   }
@@ -172,7 +181,7 @@ static double lap_at(const double *psi, int ix, int iy, int iz, int nx, int ny, 
                      const int bc[3]) {
   long x = ix + (long)nx * (iy + (long)ny * iz);
   double s = 0.0;
-  for (int i = 0; i < Q; ++i) {
+  FOR_SUM_Q(i) {
     if (Ci[i][0] == 0 && Ci[i][1] == 0 && Ci[i][2] == 0) continue;
     nbr_t nb = neighbour(ix + Ci[i][0], iy + Ci[i][1], iz + Ci[i][2], nx, ny, nz, bc);
     s += Wi[i] * (psi[nb.idx] - psi[x]);
@@ -185,7 +194,7 @@ static double lap_at(const double *psi, int ix, int iy, int iz, int nx, int ny, 
 static double div_at(const double *G3, long N, int ix, int iy, int iz, int nx, int ny, int nz,
                      const int bc[3], int rule) {
   double s = 0.0;
-  for (int i = 0; i < Q; ++i) {
+  FOR_SUM_Q(i) {
     nbr_t nb = neighbour(ix + Ci[i][0], iy + Ci[i][1], iz + Ci[i][2], nx, ny, nz, bc);
     for (int al = 0; al < 3; ++al)
       s += Wi[i] * Ci[i][al] * ghost_sign(&nb, al, rule) * G3[al * N + nb.idx];
@@ -417,7 +426,7 @@ static void pass_moments(tslb_ref *h) {
         double fi[Q];
         for (int i = 0; i < Q; ++i) fi[i] = h->f[i * N + x];
         double pst = 0.0, m[3] = {0, 0, 0}, Pi[3][3] = {{0}};
-        for (int i = 0; i < Q; ++i) {
+        FOR_SUM_Q(i) {
           pst += fi[i];                                                     /* Eq. 11 */
           for (int al = 0; al < 3; ++al) {
             m[al] += fi[i] * Ci[i][al];
@@ -435,7 +444,7 @@ static void pass_moments(tslb_ref *h) {
         double feq[Q], S[Q], A[3][3] = {{0}};
         tslb_ref_feq(pst, u, feq);
         tslb_ref_forcing(u, a, S);
-        for (int i = 0; i < Q; ++i)                                        /* Eq. 13 */
+        FOR_SUM_Q(i)                                        /* Eq. 13 */
           for (int al = 0; al < 3; ++al)
             for (int be = 0; be < 3; ++be)
               A[al][be] += H2[i][al][be] * (fi[i] - (feq[i] - 0.5 * S[i]));

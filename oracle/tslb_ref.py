@@ -19,20 +19,25 @@ _LIB = os.path.join(_HERE, "libtslb_ref.so")
 # --twin-fma to measure how far two correct roundings of this oracle drift apart.  Expected
 # values always come from the contraction-off build.
 _LIB_FMA = os.path.join(_HERE, "libtslb_ref_fma.so")
+# Second conditioning twin: the same source with every sum over the 27 directions taken in
+# reverse order (TSLB_REF_REV=1, -DTSLB_REF_REVERSE_SUMS, make_golden.py --twin-rev).
+_LIB_REV = os.path.join(_HERE, "libtslb_ref_rev.so")
 
 PERIODIC, WALL = 0, 1
 
 
-def build_lib(force=False, fma=False):
+def build_lib(force=False, fma=False, rev=False):
     """gcc -O3, contraction off (R22), OpenMP over nodes.  No -march flag: the .so travels.
     fma=True builds the conditioning twin (contraction on, -mfma) next to it."""
     hdr = os.path.join(_HERE, "tslb_ref.h")
-    out = _LIB_FMA if fma else _LIB
+    out = _LIB_FMA if fma else (_LIB_REV if rev else _LIB)
     if (not force and os.path.exists(out)
             and os.path.getmtime(out) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
         return out
     tmp = out + f".{os.getpid()}.tmp"        # build aside, then rename: a process that has the
     flags = ["-ffp-contract=fast", "-mfma"] if fma else ["-ffp-contract=off"]
+    if rev:
+        flags.append("-DTSLB_REF_REVERSE_SUMS")
     subprocess.check_call(["gcc", "-O3"] + flags + ["-fopenmp", "-fPIC", "-shared",
                            "-Wall", "-o", tmp, _SRC, "-lm"])       # old library mapped keeps it
     os.replace(tmp, out)
@@ -63,7 +68,8 @@ _dp = C.POINTER(C.c_double)
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(build_lib(fma=os.environ.get("TSLB_REF_FMA") == "1"))
+        _lib = C.CDLL(build_lib(fma=os.environ.get("TSLB_REF_FMA") == "1",
+                                rev=os.environ.get("TSLB_REF_REV") == "1"))
         _lib.tslb_ref_create.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(Params),
                                          C.POINTER(C.c_void_p)]
         _lib.tslb_ref_init.argtypes = [C.c_void_p, _dp, _dp]

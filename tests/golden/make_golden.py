@@ -12,7 +12,9 @@ Usage:  python tests/golden/make_golden.py [--twin | --twin-only [--perturb-u]] 
         oracle source built with FMA contraction on (oracle/tslb_ref.py, TSLB_REF_FMA=1) and
         store fma_<cp> = its distance from the stored expected values: two correct roundings of
         one program, differing at every multiply-add of every step, which is what a CUDA kernel
-        with another summation order is too)
+        with another summation order is too);
+        --twin-rev [case ...]: the same with the oracle source built to take every sum over the
+        27 directions in reverse order (TSLB_REF_REV=1): stores rev_<cp>)
 
 For each case the oracle runs the seeded input of paper_2501_00846_b200.inputs for the
 config's full step count and stores, at the checkpoints {1, 10, 100, 1000, ..., final}:
@@ -43,6 +45,8 @@ sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 
 if "--twin-fma" in sys.argv:
     os.environ["TSLB_REF_FMA"] = "1"                   # before the oracle library is loaded
+if "--twin-rev" in sys.argv:
+    os.environ["TSLB_REF_REV"] = "1"
 from oracle import tslb_ref as R                      # noqa: E402
 from paper_2501_00846_b200 import inputs as I          # noqa: E402
 
@@ -116,9 +120,10 @@ def run(name):
         twin.close()
 
 
-def run_twin_fma(name):
-    """Add fma_<cp> to an existing golden file (the expected values are left untouched)."""
-    assert os.environ.get("TSLB_REF_FMA") == "1"
+def run_twin_fma(name, key="fma"):
+    """Add fma_<cp> (or rev_<cp>) to an existing golden file (the expected values are left
+    untouched): the distance of a differently ROUNDED build of the same oracle source."""
+    assert os.environ.get("TSLB_REF_FMA") == "1" or os.environ.get("TSLB_REF_REV") == "1"
     make, checkpoints = cases()[name]
     path = os.path.join(HERE, name + ".npz")
     cfg = make()
@@ -134,10 +139,10 @@ def run_twin_fma(name):
         out = dict(np.load(path))                    # re-read: another twin may be writing too
         got = (rho.ravel()[idx], p.ravel()[idx], u.reshape(3, -1)[:, idx], phi.ravel()[idx])
         want = (out[f"rho_{cp}"], out[f"p_{cp}"], out[f"u_{cp}"], out[f"phi_{cp}"])
-        out[f"fma_{cp}"] = np.array([np.abs(a - b).max() / m
-                                     for a, b, m in zip(got, want, out[f"max_{cp}"])])
-        print(f"{name}: fma twin step {cp} after {time.time() - t0:.0f} s, drift = {out[f'fma_{cp}']}",
-              flush=True)
+        out[f"{key}_{cp}"] = np.array([np.abs(a - b).max() / m
+                                       for a, b, m in zip(got, want, out[f"max_{cp}"])])
+        print(f"{name}: {key} twin step {cp} after {time.time() - t0:.0f} s, drift = "
+              f"{out[f'{key}_{cp}']}", flush=True)
         np.savez_compressed(path, **out)
     twin.close()
 
@@ -179,6 +184,8 @@ if __name__ == "__main__":
     for nm in (names or list(cases())):
         if "--twin-fma" in sys.argv:
             run_twin_fma(nm)
+        elif "--twin-rev" in sys.argv:
+            run_twin_fma(nm, key="rev")
         elif "--twin-only" in sys.argv:
             run_twin_only(nm)
         else:
