@@ -2,12 +2,20 @@
 """bench.py -- GLUPS of the TSLB + Allen-Cahn step on one B200 (BASELINE.json metric).
 
 A "step" is one tslb_step(1): every stage of SURVEY.md 8(a) over the whole 256^3 head-on
-collision domain (BASELINE.json configs[3], synthetic, seeded).  `value` is timed with CUDA
-events on the solver's stream with the state resident in HBM; `e2e` goes through the C ABI's
-host-buffer calls (tslb_init_host -> tslb_step -> tslb_get_host) with the copies inside the
-timed region.  Multi-GPU = independent replicas: weak scaling, no
-data-path collective.  `--impl reference` times the CPU oracle on a bounded slab of the same
-workload (it is a deliberately plain program: context, not a target).
+collision domain (BASELINE.json configs[3], synthetic, seeded).  Protocol:
+W warm-up steps, then R repeats of exactly K steps, each between two CUDA events on the solver's
+stream with a barrier + synchronize on both sides (max over ranks per repeat); `value` comes
+from the MEDIAN repeat, the minimum is reported beside it.  The state (3.8 GB in fp64) is far
+larger than the 126 MB L2, so every step streams from HBM.  `e2e` goes through the C ABI's
+host-buffer calls (tslb_init_host -> tslb_step -> tslb_get_host) with the copies inside the timed
+region.  Multi-GPU = independent replicas: weak scaling, no data-path
+collective.  `--impl reference` times the CPU oracle on a bounded slab of the same workload (a
+deliberately plain program: context, not a target).
+
+roofline.frac follows SURVEY.md 8(d): ALGORITHMIC bytes (14 scalars read + 14 written per update)
+over the whole step's time, against the measured HBM copy rate; the per-kernel split is under
+roofline.kernels.  roofline.alu_frac is the other side of the ridge: ~0.9 kflop per update
+against the FMA throughput measured in this run (tslb_fma_peak).
 """
 import argparse
 import json
@@ -24,11 +32,13 @@ sys.path.insert(0, ROOT)
 
 METRIC = "GLUPS per B200 (fp32/fp64) and % of HBM roofline on 256^3 droplet domain"
 STATE_SCALARS = 14                      # p*, u(3), Ahat(6), a(3), phi  -> 28 s bytes per update
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel on the 256^3
-# workload, from the ncu --set full captures summarised in profiles/r1d_kernels_f64.txt and
-# profiles/r1c_kernels_f32.txt
-NCU_TRAFFIC = {("f64", "stream_collide"): 2.005029e9 + 2.102657e9,
-               ("f32", "stream_collide"): 0.977743e9 + 1.031000e9}
+FLOP_PER_UPDATE = 900.0                 # 0.8-1.0 kflop with every node quantity
+                                        # computed once (a1 70, a2 150, a4 100, a5 300, a6-a9 250)
+# dram__bytes_read.sum + dram__bytes_write.sum per STEP (all kernels of one step) on the 256^3
+# collision workload, copied from the ncu --set full captures named beside them (not measured by
+# this run: ncu cannot run inside a timed bench)
+NCU_TRAFFIC = {"f64": (4.79e9, "profiles/r1d_kernels_f64.txt"),
+               "f32": (2.40e9, "profiles/r1c_kernels_f32.txt")}
 
 
 def parse():
@@ -36,17 +46,18 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--repeats", type=int, default=5, help="timed repeats of --steps steps")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--size", type=int, default=256, help="cube edge of the domain")
-    ap.add_argument("--workload", default="collision", choices=["collision", "emulsion"],
+    ap.add_argument("--workload", default="collision",
+                    choices=["collision", "emulsion", "bubble", "offaxis"],
                     help="collision = BASELINE.json configs[3] (the graded one); emulsion = "
-                         "configs[4], the throughput sweep (use --size 384 for f64, 512 for f32)")
+                         "configs[4] (--size 384 for f64, 512 for f32); bubble = configs[2] "
+                         "(128x128x256, walls in z; --size scales it); offaxis = NEXT-2")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
                     help="precision of the headline value (the other one is reported beside it)")
-    ap.add_argument("--naive", action="store_true", help="time the validation kernels instead")
-    ap.add_argument("--variant", type=int, default=0, help="tuning variant (flags bits 8-15)")
-    ap.add_argument("--k1variant", type=int, default=0, help="Allen-Cahn tuning variant (bits 16-19)")
-    ap.add_argument("--generic", action="store_true", help="force the wall-capable tiled kernel")
+    ap.add_argument("--flags", type=int, default=0,
+                    help="validation selector (include/tslb.h TSLB_FLAG_*), 0 = production")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--only", default=None, choices=[None, "f64", "f32"],
@@ -59,53 +70,64 @@ def peaks():
     B200_PROFILING.md."""
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            return float(json.load(f)["hbm_gbs"]), "measured"
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
-        return 6650.0, "fallback"
+        return 6650.0, "fallback (B200_PROFILING.md)"
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons DURING the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """SM clock, power and throttle reasons sampled IN PROCESS through NVML at ~200 Hz for the
+    whole timed region (nvidia-smi -lms 100 in a child process missed 20 ms regions)."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+               0x4: "sw_power_cap"}
 
     def __init__(self, index):
-        self.rows, self.proc, self.index = [], None, index
+        self.index, self.rows, self.stop_flag, self.thread, self.h = index, [], False, None, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(phys)
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv, h = self.nv, self.h
+        while not self.stop_flag:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)
+                try:
+                    rs = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:
+                    rs = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                pw = nv.nvmlDeviceGetPowerUsage(h) / 1000.0
+                self.rows.append((sm, rs, pw))
+            except Exception:
+                pass
+            time.sleep(0.004)
 
     def start(self):
-        try:
-            self.proc = subprocess.Popen(
-                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                 "--format=csv,noheader,nounits", "-lms", "100"],
-                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
-        except Exception:
-            self.proc = None
-
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+        if self.nv is None:
+            return
+        self.thread = threading.Thread(target=self._loop, daemon=True)
+        self.thread.start()
 
     def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        self.t.join(timeout=2)
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
-            try:
-                sm.append(float(r[0])); mx.append(float(r[1]))
-            except Exception:
-                continue
-            for nme, v in zip(names, r[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(nme)
+        if self.nv is None or self.thread is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "samples": 0, "reasons": ["nvml unavailable"]}
+        self.stop_flag = True
+        self.thread.join(timeout=2)
+        try:
+            mx = float(self.nv.nvmlDeviceGetMaxClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+        except Exception:
+            mx = None
+        sm = [r[0] for r in self.rows]
+        reasons = sorted({name for r in self.rows for bit, name in self.REASONS.items() if r[1] & bit})
         return {"sm_mhz": float(np.median(sm)) if sm else None,
-                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
-                "reasons": sorted(reasons)}
+                "sm_min_mhz": float(min(sm)) if sm else None, "sm_max_mhz": mx,
+                "power_w_max": max((r[2] for r in self.rows), default=None),
+                "samples": len(sm), "reasons": reasons}
 
 
 def make_workload(size, kind="collision"):
@@ -113,6 +135,11 @@ def make_workload(size, kind="collision"):
     if kind == "emulsion":
         return I.emulsion_sweep(n=size)
     s = size / 256.0
+    if kind == "bubble":                 # configs[2] is 128 x 128 x 256 = --size 256
+        return I.rising_bubble(nx=int(128 * s), ny=int(128 * s), nz=int(256 * s),
+                               radius=16.0 * s, height=40.0 * s)
+    if kind == "offaxis":
+        return I.off_axis_collision(n=size)
     return I.head_on_collision(n=size, radius=24.0 * s, half_sep=40.0 * s)
 
 
@@ -142,6 +169,22 @@ def omp_threads():
         return os.cpu_count()
 
 
+def oracle_one_core(cfg, planes, steps):
+    """The same oracle on ONE core: a child process with OMP_NUM_THREADS=1 (the OpenMP runtime of
+    this process already has its team)."""
+    code = ("import sys, json; sys.path.insert(0, %r); import bench; "
+            "cfg = bench.make_workload(%d, %r); v, dt = bench.time_oracle(cfg, %d, %d); "
+            "print(json.dumps([v, dt]))" % (ROOT, cfg["_size"], cfg["_kind"], planes, steps))
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True,
+                             timeout=600).stdout.strip().splitlines()[-1]
+        v, dt = json.loads(out)
+        return v, dt
+    except Exception:
+        return None, None
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle on a bounded slab, same metric / unit / config."""
     rank = int(os.environ.get("RANK", "0"))
@@ -154,7 +197,7 @@ def run_reference(args):
     planes = int(budget * rate * 1e9 / (nx * ny * max(1, args.steps + args.warmup)))
     planes = max(4, min(nz, planes))
     glups, dt = time_oracle(cfg, planes, args.steps, args.warmup)
-    sample = f"central {nx}x{ny}x{planes} slab of the {nx}^3 input, {args.steps} steps"
+    sample = f"central {nx}x{ny}x{planes} slab of the {nx}x{ny}x{nz} input, {args.steps} steps"
     line = {"impl": "reference", "metric": METRIC, "value": glups, "unit": "GLUPS",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
@@ -168,40 +211,47 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def measure(cfg, precision, args, device, flags, dist_barrier):
-    """W warm-up steps, then exactly K steps between a barrier + synchronize on both sides.
-    Returns whole-step ms, per-kernel ms, launches, clocks."""
+def measure(cfg, precision, args, device, ranks):
+    """W warm-up steps, then R repeats of exactly K steps between a barrier + synchronize on both
+    sides; one more K-step pass with an event after every kernel gives the per-kernel split."""
     import torch
     from paper_2501_00846_b200 import binding as B
     nz, ny, nx = cfg["shape"]
-    s = B.Solver(nx, ny, nz, cfg["params"], precision=precision, flags=flags, device=device)
+    s = B.Solver(nx, ny, nz, cfg["params"], precision=precision, flags=args.flags, device=device)
     s.init(cfg["phi"], cfg["u"])
+    d0 = s.diag()
     s.step(args.warmup)
     torch.cuda.synchronize(device)
-    dist_barrier()
     sampler = ClockSampler(torch.device(device).index or 0)
     sampler.start()
     l0 = s.launches
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize(device)
-    e0.record(s.stream)
-    kernel_ms = s.step_timed(args.steps)           # events around every kernel, same stream
-    e1.record(s.stream)
-    torch.cuda.synchronize(device)
-    dist_barrier()
+    reps = []
+    for _ in range(max(1, args.repeats)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(device)
+        ranks.barrier()
+        e0.record(s.stream)
+        s.step(args.steps)
+        e1.record(s.stream)
+        torch.cuda.synchronize(device)
+        ranks.barrier()
+        reps.append(ranks.max(e0.elapsed_time(e1)))
+    launches = (s.launches - l0) // max(1, args.repeats)
     clocks = sampler.stop()
-    ms = e0.elapsed_time(e1)
-    launches = s.launches - l0
-    # sanity of the timed run: finite fields, phi conserved (P7)
-    g = s.get(("phi", "u"))
-    ok = bool(torch.isfinite(g["phi"]).all()) and bool(torch.isfinite(g["u"]).all())
-    drift = abs(float(g["phi"].double().sum()) / float(cfg["phi"].sum()) - 1.0)
+    kernel_ms = s.step_timed(args.steps)           # events around every kernel, same stream
+    # sanity of the timed run through the on-device reductions (no field is read back):
+    # finite fields, phi conserved (P7)
+    d1 = s.diag()
+    ok = all(np.isfinite(v) for v in d1.values())
+    drift = abs(d1["sum_phi"] / d0["sum_phi"] - 1.0)
     s.close()
-    return dict(ms=ms, kernel_ms=kernel_ms, launches=launches, clocks=clocks, finite=ok,
-                phi_drift=drift)
+    fma = B.tslb_fma_peak(precision)
+    return dict(ms=float(np.median(reps)), ms_min=float(min(reps)), reps=reps, kernel_ms=kernel_ms,
+                launches=launches, clocks=clocks, finite=ok, phi_drift=drift, max_u=d1["max_u"],
+                fma_tflops=fma)
 
 
-def measure_e2e(cfg, precision, args, device, flags):
+def measure_e2e(cfg, precision, args, device):
     """Host buffers through the C ABI: tslb_init_host (H2D) -> tslb_step(K) -> tslb_get_host (D2H),
     all inside the timed region."""
     import torch
@@ -212,7 +262,7 @@ def measure_e2e(cfg, precision, args, device, flags):
     u = torch.from_numpy(cfg["u"]).to(dt).pin_memory()
     out = {"rho": torch.empty_like(phi).pin_memory(), "p": torch.empty_like(phi).pin_memory(),
            "u": torch.empty_like(u).pin_memory(), "phi": torch.empty_like(phi).pin_memory()}
-    s = B.Solver(nx, ny, nz, cfg["params"], precision=precision, flags=flags, device=device)
+    s = B.Solver(nx, ny, nz, cfg["params"], precision=precision, flags=args.flags, device=device)
     s.init_host(phi, u)                            # warm-up of the copy path and the kernels
     s.step(3)
     s.get_host(out)
@@ -270,6 +320,34 @@ def whole_job_glups(nodes, steps, ms_max, world):
     return world * nodes * steps / (ms_max * 1e-3) / 1e9
 
 
+def roofline(r, prec, n, steps, peak, peak_kind, periodic_fast, full_size):
+    """frac = algorithmic bytes (28 s per update) over the step time, against the
+    measured copy rate.  Per kernel: its own duration and the scalars it really moves."""
+    es = 8 if prec == "f64" else 4
+    ms_step = r["ms"] / steps
+    b_alg = 2 * STATE_SCALARS * es
+    ach = b_alg * n / (ms_step * 1e-3) / 1e9
+    dom = max(r["kernel_ms"], key=r["kernel_ms"].get)
+    moved = ({"stream_collide": 30, "allen_cahn": 5} if periodic_fast
+             else {"stream_collide": 27, "allen_cahn": 8, "normal": 4})
+    tot_k = sum(r["kernel_ms"].values())
+    kernels = {k: {"ms": v / steps, "share_of_step": v / tot_k,
+                   "moved_scalars_per_update": moved.get(k),
+                   "moved_gbs": moved[k] * es * n / (v / steps * 1e-3) / 1e9 if k in moved else None}
+               for k, v in r["kernel_ms"].items()}
+    traffic, src = NCU_TRAFFIC.get(prec, (None, None)) if (periodic_fast and full_size) else (None, None)
+    alu_ach = FLOP_PER_UPDATE * n / (ms_step * 1e-3) / 1e12
+    return {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
+            "frac": ach / peak, "frac_min_repeat": b_alg * n / (r["ms_min"] / steps * 1e-3) / 1e9 / peak,
+            "frac_of_8TBs": ach / 8000.0, "traffic": traffic, "traffic_source": src,
+            "traffic_unit": "bytes per step (all kernels), ncu dram__bytes_read+write",
+            "peak_kind": peak_kind, "algorithmic_bytes_per_update": b_alg,
+            "kernels": kernels,
+            "alu_frac": alu_ach / r["fma_tflops"], "alu_achieved_tflops": alu_ach,
+            "alu_peak_tflops": r["fma_tflops"], "alu_flop_per_update": FLOP_PER_UPDATE,
+            "alu_peak_kind": "measured in this run (tslb_fma_peak, dependent-chain-free FMA)"}
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -278,75 +356,65 @@ def main():
     ranks = Ranks("nccl")
     world, rank, device = ranks.world, ranks.rank, ranks.device
     torch.cuda.set_device(ranks.local)
-    barrier, max_over_ranks = ranks.barrier, ranks.max
 
-    flags = (1 if args.naive else 0) | (2 if args.generic else 0) | (args.variant << 8) | (args.k1variant << 16)
     cfg = make_workload(args.size, args.workload)
+    cfg["_size"], cfg["_kind"] = args.size, args.workload
     n = int(np.prod(cfg["shape"]))
     peak, peak_kind = peaks()
     order = [args.only] if args.only else [args.precision, "f32" if args.precision == "f64" else "f64"]
+    periodic_fast = not (args.flags & 3) and not any(cfg["params"]["bc"])
+    full = args.workload == "collision" and args.size == 256
     res = {}
     for prec in order:
-        r = measure(cfg, prec, args, device, flags, barrier)
-        r["ms"] = max_over_ranks(r["ms"])
-        es = 8 if prec == "f64" else 4
+        r = measure(cfg, prec, args, device, ranks)
         r["glups"] = whole_job_glups(n, args.steps, r["ms"], world)
-        # dominant kernel and its roofline: algorithmic bytes of the
-        # whole update, 28 s per node, charged to the dominant kernel's own duration only when
-        # the step is a single kernel; for a split step each kernel is charged its own planes.
-        dom = max(r["kernel_ms"], key=r["kernel_ms"].get)
-        # scalars per update the dominant kernel must move: the periodic
-        # stream-collide kernel reads 13 moments + phi^{n+1} and writes 13 moments + the flux Q (3);
-        # the wall-capable / naive one writes no Q.
-        periodic_fast = not (args.naive or args.generic) and not any(cfg["params"]["bc"])
-        planes = {"stream_collide": 30 if periodic_fast else 27, "allen_cahn": 5, "normal": 4}[dom]
-        k_ms = r["kernel_ms"][dom] / args.steps
-        ach = planes * es * n / (k_ms * 1e-3) / 1e9
-        step_ach = 2 * STATE_SCALARS * es * n / (r["ms"] / args.steps * 1e-3) / 1e9
-        r["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak,
-                         "unit": "GB/s", "frac": ach / peak,
-                         "traffic": NCU_TRAFFIC.get((prec, dom)) if (periodic_fast and n == 256 ** 3) else None,
-                         "peak_kind": peak_kind, "kernel_ms": k_ms,
-                         "kernels_ms": {k: v / args.steps for k, v in r["kernel_ms"].items()},
-                         "kernel_share_of_step": r["kernel_ms"][dom] / r["ms"],
-                         "algorithmic_bytes_per_update": planes * es,
-                         "step_achieved": step_ach, "step_frac": step_ach / peak,
-                         "step_frac_of_8TBs": step_ach / 8000.0}
+        r["roofline"] = roofline(r, prec, n, args.steps, peak, peak_kind, periodic_fast, full)
+        if not args.no_e2e:
+            r["e2e"] = measure_e2e(cfg, prec, args, device)
+            r["e2e"]["value"] *= world
         res[prec] = r
     head = res[order[0]]
-    e2e = None
-    if not args.no_e2e:
-        e2e = measure_e2e(cfg, order[0], args, device, flags)
-        e2e["value"] = world * e2e["value"] if world > 1 else e2e["value"]
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         planes, osteps = min(64, cfg["shape"][0]), 8
         v, dt = time_oracle(cfg, planes, osteps)
-        cpu = {"value": v, "unit": "GLUPS", "cores": omp_threads(), "kind": "oracle",
-               "sample": f"central {cfg['shape'][2]}x{cfg['shape'][1]}x{planes} slab of the same "
-                         f"input, {osteps} steps, {dt:.1f} s"}
+        sample = (f"central {cfg['shape'][2]}x{cfg['shape'][1]}x{planes} slab of the same input, "
+                  f"{osteps} steps, {dt:.1f} s")
+        cpu = {"value": v, "unit": "GLUPS", "cores": omp_threads(), "kind": "oracle", "sample": sample}
+        v1, dt1 = oracle_one_core(cfg, min(8, cfg["shape"][0]), 2)
+        if v1 is not None:
+            cpu["one_core"] = {"value": v1, "unit": "GLUPS", "cores": 1,
+                               "sample": f"central slab of {min(8, cfg['shape'][0])} planes, 2 steps, {dt1:.1f} s"}
     if rank == 0:
+        es0 = 8 if order[0] == "f64" else 4
         line = {"metric": METRIC, "value": head["glups"], "unit": "GLUPS", "n_gpus": world,
-                "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": head["ms"] / args.steps, "higher_is_better": True,
+                "steps": args.steps, "warmup": args.warmup, "repeats": args.repeats,
+                "ms_per_step": head["ms"] / args.steps,
+                "ms_per_step_min": head["ms_min"] / args.steps,
+                "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": order[0], "data": "synthetic",
                 "config": {"workload": cfg["name"], "grid": list(cfg["shape"][::-1]),
                            "parallelism": f"replicas x{world}",
-                           "l2": f"state {2 * STATE_SCALARS * (8 if order[0] == 'f64' else 4) * n / 1e9:.1f} GB ({order[0]}) >> 126 MB L2",
-                           "path": "naive" if args.naive else ("tiled-generic" if args.generic else "tiled"),
-                           "variant": args.variant},
+                           "l2": f"state {2 * STATE_SCALARS * es0 * n / 1e9:.1f} GB ({order[0]}) >> 126 MB L2: "
+                                 "inputs larger than L2, no flush needed",
+                           "flags": args.flags,
+                           "timing": f"median of {args.repeats} repeats of {args.steps} steps (CUDA events)"},
                 "clocks": head["clocks"], "gpu_launches": head["launches"],
                 "roofline": head["roofline"], "finite": head["finite"],
-                "phi_drift": head["phi_drift"]}
-        if e2e:
-            line["e2e"] = e2e
+                "phi_drift": head["phi_drift"], "max_u": head["max_u"]}
+        if "e2e" in head:
+            line["e2e"] = head["e2e"]
         if cpu:
             line["cpu_baseline"] = cpu
         for prec in order[1:]:
             o = res[prec]
             line[prec] = {"value": o["glups"], "unit": "GLUPS", "ms_per_step": o["ms"] / args.steps,
+                          "ms_per_step_min": o["ms_min"] / args.steps,
                           "roofline": o["roofline"], "clocks": o["clocks"],
-                          "gpu_launches": o["launches"], "finite": o["finite"]}
+                          "gpu_launches": o["launches"], "finite": o["finite"],
+                          "phi_drift": o["phi_drift"]}
+            if "e2e" in o:
+                line[prec]["e2e"] = o["e2e"]
         print(json.dumps(line), flush=True)
     ranks.close()
 

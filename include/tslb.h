@@ -38,15 +38,20 @@ enum { TSLB_BC_PERIODIC = 0, TSLB_BC_WALL = 1 }; /* per axis, both ends (P:264, 
 enum { TSLB_F32 = 0, TSLB_F64 = 1 };
 enum { TSLB_OK = 0, TSLB_EINVAL = -1, TSLB_EWORKSPACE = -2, TSLB_ECUDA = -3, TSLB_ESTATE = -4 };
 
-/* flags (bit field) */
+/* flags (bit field): validation selectors.  0 = the library chooses (production).  Every flag
+ * forces another kernel of the product that computes the SAME step (same arithmetic contract,
+ * same tolerances); there are no tuning or timing variants behind this field and any other bit
+ * makes tslb_create fail with TSLB_EINVAL. */
 enum {
-  TSLB_FLAG_NAIVE = 1,   /* run the one-thread-per-node global-memory kernels (debug/validation
-                            path, same arithmetic contract); default 0 = tiled z-marching kernels */
-  TSLB_FLAG_GENERIC = 2, /* on an all-periodic box, run the wall-capable tiled kernel instead of
-                            the lean periodic one (validation of the former at full size)        */
-  TSLB_FLAG_VARIANT_MASK = 0xff00 /* bits 8-15: tuning variant of the lean kernel (tile height,
-                            blocks per SM, prefetch), bits 16-23: of the Allen-Cahn kernel;
-                            0 = the production choice                                            */
+  TSLB_FLAG_NAIVE = 1,      /* one-thread-per-node global-memory kernels (validation path)        */
+  TSLB_FLAG_GENERIC = 2,    /* on an all-periodic box, the wall-capable tiled pair                */
+  TSLB_FLAG_K2_CPASYNC = 4, /* lean periodic stream-collide kernel with cp.async staging, even
+                               where the TMA-staged one would be chosen                           */
+  TSLB_FLAG_K2_TMA = 8,     /* ... with TMA tensor staging wherever it is usable (nx % 32 == 0,
+                               nx >= 64, ny > 8), even where cp.async would be chosen            */
+  TSLB_FLAG_K1_FLUX = 16,   /* one-node-per-thread flux-form interface kernel instead of the row
+                               kernel                                                             */
+  TSLB_FLAG_ALL = 31
 };
 
 typedef struct tslb_params {
@@ -143,6 +148,12 @@ enum { TSLB_K_NORMAL = 0,          /* naive path only: sharpening-flux kernel   
        TSLB_K_STREAM_COLLIDE = 2,  /* fused stream-collide-moments-forces, Eq. 7-17       */
        TSLB_NKERNELS = 4 };
 int tslb_step_timed(tslb_handle *h, int n, float *kernel_ms);
+
+/* ALU side of the roofline: measured throughput, in TFLOP/s (2 flops per FMA), of
+ * dependent-chain-free fused multiply-adds in the given precision on the current device, timed
+ * with CUDA events on `stream` (synchronises).  A micro-benchmark for bench.py's
+ * roofline.alu_frac, not part of the path; needs no handle and allocates nothing. */
+int tslb_fma_peak(int precision, void *stream, double *tflops);
 
 /* Number of kernel launches the handle has enqueued so far (for bench.py's gpu_launches). */
 long long tslb_launch_count(const tslb_handle *h);

@@ -13,7 +13,7 @@ LIB_PATH = os.path.join(_HERE, "libtslb.so")
 
 BC_PERIODIC, BC_WALL = 0, 1
 F32, F64 = 0, 1
-FLAG_NAIVE = 1
+FLAG_NAIVE, FLAG_GENERIC, FLAG_K2_CPASYNC, FLAG_K2_TMA, FLAG_K1_FLUX = 1, 2, 4, 8, 16
 NDIAG = 16
 DIAG_NAMES = ("sum_phi", "sum_pstar", "max_u", "sum_phi_x", "sum_phi_y", "sum_phi_z",
               "sum_phi_ux", "sum_phi_uy", "sum_phi_uz", "sum_ux", "sum_uy", "sum_uz",
@@ -21,7 +21,7 @@ DIAG_NAMES = ("sum_phi", "sum_pstar", "max_u", "sum_phi_x", "sum_phi_y", "sum_ph
 
 SYMBOLS = ("tslb_workspace_bytes", "tslb_create", "tslb_init", "tslb_step", "tslb_get",
            "tslb_get_state", "tslb_init_host", "tslb_get_host", "tslb_step_timed",
-           "tslb_launch_count", "tslb_diag", "tslb_diag_host", "tslb_diag_static",
+           "tslb_launch_count", "tslb_diag", "tslb_diag_host", "tslb_diag_static", "tslb_fma_peak",
            "tslb_destroy", "tslb_last_error")
 
 
@@ -71,6 +71,7 @@ def load():
     lib.tslb_diag.argtypes = [vp, vp]
     lib.tslb_diag_host.argtypes = [vp, C.POINTER(C.c_double)]
     lib.tslb_diag_static.argtypes = [vp, vp]
+    lib.tslb_fma_peak.argtypes = [C.c_int, vp, C.POINTER(C.c_double)]
     lib.tslb_launch_count.argtypes = [vp]
     lib.tslb_launch_count.restype = C.c_longlong
     lib.tslb_destroy.argtypes = [vp]
@@ -91,6 +92,15 @@ def _check(rc, what):
 
 def tslb_workspace_bytes(nx, ny, nz, params):
     return int(load().tslb_workspace_bytes(nx, ny, nz, C.byref(params)))
+
+
+def tslb_fma_peak(precision="f64", stream=None):
+    """Measured FMA throughput (TFLOP/s) of the plain ALUs on the current device."""
+    out = C.c_double()
+    _check(load().tslb_fma_peak(F64 if precision == "f64" else F32,
+                                stream.cuda_stream if stream is not None else None,
+                                C.byref(out)), "tslb_fma_peak")
+    return float(out.value)
 
 
 class Solver:
@@ -126,6 +136,12 @@ class Solver:
                                     self.stream.cuda_stream, C.byref(self._h)), "tslb_create")
 
     # -- helpers -------------------------------------------------------------------------
+    def _call(self, name, *args):
+        """One ABI call with the solver's device current (launch attributes, the static scratch
+        of tslb_diag_static and the stream all belong to a device)."""
+        with self.torch.cuda.device(self.device):
+            _check(getattr(self.lib, name)(self._h, *args), name)
+
     def _dev(self, a, shape):
         t = self.torch.as_tensor(a)
         t = t.to(device=self.device, dtype=self.dtype).contiguous()
@@ -140,51 +156,49 @@ class Solver:
         """tslb_init from device tensors (host arrays are copied to the device by torch first)."""
         phi = self._dev(phi, self.shape)
         u = self._dev(u, (3,) + self.shape)
-        with self.torch.cuda.stream(self.stream):
-            _check(self.lib.tslb_init(self._h, phi.data_ptr(), u.data_ptr()), "tslb_init")
+        self._call("tslb_init", phi.data_ptr(), u.data_ptr())
         self.stream.synchronize()          # phi, u may be temporaries
 
     def init_host(self, phi, u):
         """tslb_init_host from host arrays/tensors of the solver's precision (pinned = async)."""
         phi, u = self._host_ptr(phi, self.shape), self._host_ptr(u, (3,) + self.shape)
-        _check(self.lib.tslb_init_host(self._h, phi[1], u[1]), "tslb_init_host")
+        self._call("tslb_init_host", phi[1], u[1])
         self.stream.synchronize()
         return self
 
     def step(self, n=1):
-        _check(self.lib.tslb_step(self._h, int(n)), "tslb_step")
+        self._call("tslb_step", int(n))
 
     def step_timed(self, n=1):
         """tslb_step_timed: returns {kernel kind: total ms over the n steps} (synchronises)."""
         ms = (C.c_float * 4)()
-        _check(self.lib.tslb_step_timed(self._h, int(n), ms), "tslb_step_timed")
+        self._call("tslb_step_timed", int(n), ms)
         names = ("normal", "allen_cahn", "stream_collide", "reserved")
         return {k: float(v) for k, v in zip(names, ms) if v > 0.0}
 
     def get(self, want=("rho", "p", "u", "phi")):
         out = {k: (self._empty(3) if k == "u" else self._empty()) for k in want}
         ptr = lambda k: out[k].data_ptr() if k in out else None
-        _check(self.lib.tslb_get(self._h, ptr("rho"), ptr("p"), ptr("u"), ptr("phi")), "tslb_get")
+        self._call("tslb_get", ptr("rho"), ptr("p"), ptr("u"), ptr("phi"))
         return out
 
     def get_state(self):
         out = dict(pstar=self._empty(), u=self._empty(3), A=self._empty(6), a=self._empty(3),
                    phi=self._empty())
-        _check(self.lib.tslb_get_state(self._h, out["pstar"].data_ptr(), out["u"].data_ptr(),
-                                       out["A"].data_ptr(), out["a"].data_ptr(),
-                                       out["phi"].data_ptr()), "tslb_get_state")
+        self._call("tslb_get_state", out["pstar"].data_ptr(), out["u"].data_ptr(),
+                   out["A"].data_ptr(), out["a"].data_ptr(), out["phi"].data_ptr())
         return out
 
     def diag(self):
         """tslb_diag_host: dict of the TSLB_D_* box reductions (synchronises the stream)."""
         out = (C.c_double * NDIAG)()
-        _check(self.lib.tslb_diag_host(self._h, out), "tslb_diag_host")
+        self._call("tslb_diag_host", out)
         return dict(zip(DIAG_NAMES, out))
 
     def diag_device(self):
         """tslb_diag into a device tensor of NDIAG doubles (no synchronisation)."""
         out = self.torch.empty(NDIAG, dtype=self.torch.float64, device=self.device)
-        _check(self.lib.tslb_diag(self._h, out.data_ptr()), "tslb_diag")
+        self._call("tslb_diag", out.data_ptr())
         return out
 
     def diag_static(self, out=None):
@@ -194,16 +208,15 @@ class Solver:
             out = self.torch.empty(NDIAG, dtype=self.torch.float64, device=self.device)
         assert out.dtype == self.torch.float64 and out.numel() == NDIAG and out.is_contiguous()
         assert out.device == self.device
-        with self.torch.cuda.device(self.device):
-            _check(self.lib.tslb_diag_static(self._h, out.data_ptr()), "tslb_diag_static")
+        self._call("tslb_diag_static", out.data_ptr())
         return out
 
     def get_host(self, out):
         """tslb_get_host into a dict of host arrays/tensors {rho,p,u,phi} (any subset)."""
         ptrs = {k: self._host_ptr(v, ((3,) if k == "u" else ()) + self.shape)[1]
                 for k, v in out.items()}
-        _check(self.lib.tslb_get_host(self._h, ptrs.get("rho"), ptrs.get("p"), ptrs.get("u"),
-                                      ptrs.get("phi")), "tslb_get_host")
+        self._call("tslb_get_host", ptrs.get("rho"), ptrs.get("p"), ptrs.get("u"),
+                   ptrs.get("phi"))
         return out
 
     def _host_ptr(self, a, shape):

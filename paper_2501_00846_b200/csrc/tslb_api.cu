@@ -39,7 +39,7 @@ bool params_ok(int nx, int ny, int nz, const tslb_params* p) {
         p->mobility > 0 && p->sigma >= 0))
     return false;
   if (p->precision != TSLB_F32 && p->precision != TSLB_F64) return false;
-  if (p->flags & ~(TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC | TSLB_FLAG_VARIANT_MASK | 0xff0000)) return false;
+  if (p->flags & ~TSLB_FLAG_ALL) return false;   // stray bits never select anything
   const int n[3] = {nx, ny, nz};
   for (int d = 0; d < 3; ++d) {
     if (p->bc[d] != TSLB_BC_PERIODIC && p->bc[d] != TSLB_BC_WALL) return false;
@@ -191,6 +191,28 @@ int get_impl(tslb_handle* h, T* rho, T* p, T* u, long long u_stride, T* phi) {
   return TSLB_OK;
 }
 
+static __device__ double g_fma_sink[2];
+
+template <typename T, int NCHAIN, int NITER>
+__global__ void __launch_bounds__(256) k_fma_peak(T seed) {
+  T a[NCHAIN];
+#pragma unroll
+  for (int c = 0; c < NCHAIN; ++c) a[c] = seed + T(c + threadIdx.x) * T(1e-3);
+  const T m = T(0.999) + seed, b = T(1e-4);
+#pragma unroll 1
+  for (int it = 0; it < NITER; it += 8) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int c = 0; c < NCHAIN; ++c) a[c] = fma(a[c], m, b);
+    }
+  }
+  T s = 0;
+#pragma unroll
+  for (int c = 0; c < NCHAIN; ++c) s += a[c];
+  if (s == T(-12345.678)) g_fma_sink[sizeof(T) == 8] = double(s);    // never true: keeps the chains
+}
+
 }  // namespace
 
 extern "C" {
@@ -294,6 +316,44 @@ int tslb_diag_host(tslb_handle* h, double* out) {
   CUDA_TRY(cudaMemcpyAsync(out, d_out, tslb::NDIAG * sizeof(double), cudaMemcpyDeviceToHost,
                            h->stream));
   CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return TSLB_OK;
+}
+
+// ---- tslb_fma_peak: the ALU side of the roofline (SURVEY.md 8(d) "Both fractions") ------------
+// Dependent-chain-free FMA throughput of the plain ALUs, measured on the spot: every thread
+// runs NCHAIN independent fused multiply-add chains for NITER iterations (registers only), the
+// grid fills every SM several times over.  2 flops per FMA.  The result is the denominator of
+// bench.py's roofline.alu_frac; it is a micro-benchmark, not part of the path.
+int tslb_fma_peak(int precision, void* stream, double* tflops) {
+  if (!tflops || (precision != TSLB_F32 && precision != TSLB_F64))
+    return fail(TSLB_EINVAL, "tslb_fma_peak: bad argument");
+  constexpr int NCHAIN = 8, NITER = 8192, THREADS = 256;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  int dev = 0, sms = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int blocks = sms * 32;
+  cudaEvent_t e0, e1;
+  CUDA_TRY(cudaEventCreate(&e0));
+  CUDA_TRY(cudaEventCreate(&e1));
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {                    // first repetition = warm-up
+    cudaEventRecord(e0, st);
+    if (precision == TSLB_F64) k_fma_peak<double, NCHAIN, NITER><<<blocks, THREADS, 0, st>>>(1e-9);
+    else k_fma_peak<float, NCHAIN, NITER><<<blocks, THREADS, 0, st>>>(1e-9f);
+    cudaEventRecord(e1, st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (e != cudaSuccess) {
+      cudaEventDestroy(e0); cudaEventDestroy(e1);
+      return fail(TSLB_ECUDA, "tslb_fma_peak: %s", cudaGetErrorString(e));
+    }
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *tflops = 2.0 * NCHAIN * double(NITER) * THREADS * blocks / (double(best) * 1e-3) / 1e12;
   return TSLB_OK;
 }
 

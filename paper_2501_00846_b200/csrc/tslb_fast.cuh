@@ -171,22 +171,21 @@ __device__ __forceinline__ Red6<T> reduce6(const T (&v)[3][3]) {   // v[cx+1][cy
   return r;
 }
 
-// ABL != 0 : timing ablations (wrong results on purpose; never selected in production)
-//   bit mask: 1 no shared-memory reads, 2 no closing arithmetic, 4 no global stores,
-//   8 no global loads, 16 no source arithmetic (main warps), 32 no shared-memory writes
-// NSTAGE > 0 : cp.async staging NSTAGE planes ahead (PREFETCH is then ignored)
-template <typename T, int TX, int TY, int MINB, bool PREFETCH, int ABL = 0, int NSTAGE = 0>
+// cp.async staging NSTAGE >= 1 planes ahead: each thread copies the 14 scalars of ITS OWN node
+// for plane j + NSTAGE straight into a private shared-memory slot (StageBuf, tslb_device.cuh)
+// and picks them up NSTAGE iterations later; only cp.async.wait_group is needed.
+template <typename T, int TX, int TY, int MINB, int NSTAGE>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
 k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D,
                       T* __restrict__ Qout, int zchunk) {
+  static_assert(NSTAGE >= 1, "the kernel is latency-bound without staging");
   using M = TileMap<TX, TY, 1>;
   using SM = K2FastSmem<T, M::CELLS, M::NMAIN>;
   using XB = ExBuf<T, M::CELLS, M::NMAIN>;
   using STG = StageBuf<T, M::CELLS>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
-  STG* stg = reinterpret_cast<STG*>(smem_raw + sizeof(SM));      // NSTAGE slots (if any)
-  constexpr bool REGPF = PREFETCH && NSTAGE == 0;
+  STG* stg = reinterpret_cast<STG*>(smem_raw + sizeof(SM));      // NSTAGE slots
 
   const int tid = threadIdx.x;
   int lx, ly;
@@ -207,92 +206,33 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
 
   // cp.async pipeline: one commit group per plane, issued by every thread (possibly empty)
   auto stage_issue = [&](int j, int slot) {
-    if (NSTAGE > 0) {
-      if (in_ring && j <= z1 && !(ABL & 8)) {
-        using V = typename VecOf<T>::type;
-        const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
-        const int s = col + plane * jz;
-        const V* g = reinterpret_cast<const V*>(S);
+    if (in_ring && j <= z1) {
+      using V = typename VecOf<T>::type;
+      const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
+      const int s = col + plane * jz;
+      const V* g = reinterpret_cast<const V*>(S);
 #pragma unroll
-        for (int k = 0; k < 12 / VecOf<T>::W; ++k) cp_async16(&stg[slot].vec[k][c], g + k * P.N + s);
-        cp_async_small(&stg[slot].az[c], S + 12 * P.N + s);
-        cp_async_small(&stg[slot].ph[c], phin + s);
-      }
-      cp_async_commit();
+      for (int k = 0; k < 12 / VecOf<T>::W; ++k) cp_async16(&stg[slot].vec[k][c], g + k * P.N + s);
+      cp_async_small(&stg[slot].az[c], S + 12 * P.N + s);
+      cp_async_small(&stg[slot].ph[c], phin + s);
     }
+    cp_async_commit();
   };
   auto stage_take = [&](int slot, T (&m)[13], T& ph) {
     constexpr int W = VecOf<T>::W;
-    if (ABL & 8) {
-#pragma unroll
-      for (int f = 0; f < 13; ++f) m[f] = T(1e-3) * T(f + (c & 7));
-      ph = T(0.5);
-      return;
-    }
 #pragma unroll
     for (int k = 0; k < 12 / W; ++k) unpack(stg[slot].vec[k][c], &m[k * W]);
     m[12] = stg[slot].az[c];
     ph = stg[slot].ph[c];
   };
-  if (NSTAGE > 0) {
 #pragma unroll
-    for (int d = 0; d < NSTAGE; ++d) stage_issue(z0 - 1 + d, d);
-  }
+  for (int d = 0; d < NSTAGE; ++d) stage_issue(z0 - 1 + d, d);
 
   // Register pipeline along z.  Two slots alternate roles every plane ("A" = destination plane
   // j-1, completed in iteration j; "B" = destination plane j), so the marching loop is unrolled
   // by two and no register is moved to shift the pipeline.
   T acc0[6] = {}, acc1[6] = {}, zo0[3] = {}, zo1[3] = {}, u0[3] = {}, u1[3] = {};
   T ph_m = 0, ph_0 = 0, ph_p = 0;
-  T nxt[13], nxt_phi = 0;                      // prefetched state of the next source plane
-
-  auto load_plane = [&](int j, T (&m)[13], T& ph) {
-    const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
-    const int s = col + plane * jz;
-    if (ABL & 8) {
-#pragma unroll
-      for (int f = 0; f < 13; ++f) m[f] = T(1e-3) * T(f + (s & 7));
-      ph = T(0.5);
-    } else {
-      load13(S, P.N, s, m);
-      ph = __ldg(phin + s);
-    }
-  };
-  // ---- halo warps: sources only.  They have no receive phase to hide the memory latency of
-  // the next plane behind, and every main warp waits for them at the barrier, so they prefetch
-  // TWO planes ahead (registers are plentiful here: no accumulators).
-  if (REGPF && tid >= M::NMAIN) {
-    T pa[13], pb[13], fa = 0, fb = 0;
-    if (in_ring) {
-      load_plane(z0 - 1, pa, fa);
-      load_plane(z0, pb, fb);
-    }
-    for (int j = z0 - 1; j <= z1; ++j) {
-      XB& xb = sm.buf[(j - z0 + 1) & 1];
-      ph_m = ph_0; ph_0 = ph_p;
-      if (in_ring) {
-        T cur[13];
-#pragma unroll
-        for (int f = 0; f < 13; ++f) { cur[f] = pa[f]; pa[f] = pb[f]; }
-        ph_p = fa; fa = fb;
-        if (j + 2 <= z1) load_plane(j + 2, pb, fb);
-        const Coef<T> cf = coef_from13(cur);
-        SrcFields<T> sf;
-        source_fields(cf, sf);
-#pragma unroll
-        for (int q = 0; q < 9; ++q) {
-          const int cx = q % 3 - 1, cy = q / 3 - 1;
-          if (cx == 0 && cy == 0) continue;
-          if (need >> dir_slot(cx, cy) & 1u)
-            xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
-        }
-        xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
-      }
-      __syncthreads();
-    }
-    return;
-  }
-  if (REGPF && in_ring) load_plane(z0 - 1, nxt, nxt_phi);
 
   auto body = [&](const int j, const int slot, XB& xb, T (&aA)[6], T (&aB)[6],
                   T (&zA)[3], T (&zB)[3], const T (&uPrev)[3], T (&uCur)[3]) {
@@ -300,38 +240,24 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
     ph_m = ph_0; ph_0 = ph_p;
     if (in_ring) {
       T cur[13];
-      if (NSTAGE > 0) {
-        cp_async_wait<(NSTAGE > 0 ? NSTAGE - 1 : 0)>();        // the group of plane j has landed
-        stage_take(slot, cur, ph_p);
-      } else if (REGPF) {
-#pragma unroll
-        for (int f = 0; f < 13; ++f) cur[f] = nxt[f];
-        ph_p = nxt_phi;
-      } else {
-        load_plane(j, cur, ph_p);
-      }
+      cp_async_wait<NSTAGE - 1>();                             // the group of plane j has landed
+      stage_take(slot, cur, ph_p);
       uCur[0] = cur[F_UX]; uCur[1] = cur[F_UY]; uCur[2] = cur[F_UZ];
       SrcFields<T> sf;
-      if (ABL & 16) {
-#pragma unroll
-        for (int a = 0; a < 9; ++a) { sf.E[a / 3][a % 3] = cur[a]; sf.O[a / 3][a % 3] = cur[a + 2]; sf.Q[a / 3][a % 3] = cur[a + 4]; }
-      } else {
-        const Coef<T> cf = coef_from13(cur);
-        source_fields(cf, sf);
-      }
+      const Coef<T> cf = coef_from13(cur);
+      source_fields(cf, sf);
       ownE = sf.E[1][1]; ownO = sf.O[1][1]; ownQ = sf.Q[1][1];
 #pragma unroll
       for (int q = 0; q < 9; ++q) {
         const int cx = q % 3 - 1, cy = q / 3 - 1;
         if (cx == 0 && cy == 0) continue;
-        if ((need >> dir_slot(cx, cy) & 1u) && (!(ABL & 32) || cx + cy == 2))
+        if (need >> dir_slot(cx, cy) & 1u)
           xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
       }
       xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
     }
-    stage_issue(j + NSTAGE, slot);             // refill the slot just consumed (no-op if NSTAGE = 0)
+    stage_issue(j + NSTAGE, slot);             // refill the slot just consumed
     __syncthreads();
-    if (REGPF && in_ring && j < z1) load_plane(j + 1, nxt, nxt_phi);
 
     if (is_out) {
       Red6<T> rE, rO, rQ;
@@ -342,7 +268,6 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         for (int q = 0; q < 9; ++q) {
           const int cx = q % 3 - 1, cy = q / 3 - 1;
           if (cx == 0 && cy == 0) continue;
-          if ((ABL & 1) && q != 8) { vE[cx + 1][cy + 1] = ownE * T(q); vO[cx + 1][cy + 1] = ownO * T(q); continue; }
           xb.get_eo(dir_slot(cx, cy), tid, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
         }
         rE = reduce6(vE);
@@ -356,7 +281,6 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         for (int q = 0; q < 9; ++q) {
           const int cx = q % 3 - 1, cy = q / 3 - 1;
           if (cx == 0 && cy == 0) continue;
-          if ((ABL & 1) && q != 8) { vQ[cx + 1][cy + 1] = ownQ * T(q); continue; }
           xb.get_q(dir_slot(cx, cy), tid, vQ[cx + 1][cy + 1]);
         }
         rQ = reduce6(vQ);
@@ -388,12 +312,9 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         for (int r = 0; r < 3; ++r) {
           const int cc = c + (r - 1) * M::W;
           T am, a0, ap, bm, b0, bp;
-          if (ABL & 1) { am = a0 = ap = ph_0 * T(r); bm = b0 = bp = ph_p; }
-          else {
           xb.get_pd(cc - 1, am, bm);
           xb.get_pd(cc, a0, b0);
           xb.get_pd(cc + 1, ap, bp);
-          }
           rs[r] = fma(T(4), a0, am + ap);
           rd[r] = ap - am;
           zs[r] = fma(T(4), b0, bm + bp);
@@ -403,14 +324,13 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         const T gy_ = (rs[2] - rs[0]) * T(3.0 / 216.0);
         const T gz_ = fma(T(4), zs[1], zs[0] + zs[2]) * T(3.0 / 216.0);
         const T lap = fma(T(6.0 / 216.0), sw, T(-6) * ph_0);
-        NodeOut<T> out;
-        if (ABL & 2) { out.p = m.p + lap; out.ux = m.mx + gx_; out.uy = m.my + gy_; out.uz = m.mz + gz_; out.axx = m.xx; out.ayy = m.yy; out.azz = m.zz; out.axy = m.xy; out.axz = m.xz; out.ayz = m.yz; out.ax = uPrev[0]; out.ay = uPrev[1]; out.az = uPrev[2]; }
-        else out = close_node(P, m, ph_0, gx_, gy_, gz_, lap, uPrev[0], uPrev[1], uPrev[2]);
-        if (!(ABL & 4) || out.p == T(123.456)) store_out(D, P.N, gx + P.nx * gy + plane * k, out);
-        if (Qout != nullptr && !(ABL & 4)) {        // flux of Eq. 20 for the next step (K1 flux form)
+        const NodeOut<T> out = close_node(P, m, ph_0, gx_, gy_, gz_, lap, uPrev[0], uPrev[1], uPrev[2]);
+        const long long idx = gx + P.nx * gy + (long long)plane * k;
+        store_out(D, P.N, idx, out);
+        if (Qout != nullptr) {                      // flux of Eq. 20 for the next step (K1 flux form)
           T q[3];
           flux_q(P, ph_0, gx_, gy_, gz_, out.ux, out.uy, out.uz, q);
-          store_q(Qout, P.N, gx + P.nx * gy + plane * k, q);
+          store_q(Qout, P.N, idx, q);
         }
       }
       // slot A is free now: it becomes the accumulator of destination plane j+1
@@ -431,7 +351,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
       next_slot();
     }
   }
-  if (NSTAGE > 0) cp_async_wait<0>();
+  cp_async_wait<0>();
 }
 
 }  // namespace tslb

@@ -4,11 +4,11 @@
 // source planes reach shared memory.  There every thread copies the 14 scalars of its own node
 // with 8 cp.async instructions per plane; their shared-memory writes arrive sector by sector and
 // cost about three times the ideal number of wavefronts in the LSU data pipe, which the
-// population exchange already loads to ~60 % (profiles/r1b_*).  Here ONE extra warp issues
+// population exchange already loads to ~60 % (profiles/r1_tuning_evidence.md).  Here ONE extra warp issues
 // cp.async.bulk.tensor copies (TMA) for the whole ring of the tile, NSTAGE planes ahead,
 // completing on an mbarrier per staging slot:
-//   * one 4-d box (x, y, z, f) per 128-bit field-vector plane of the ring (SPLIT, production:
-//     6 boxes in fp64; a single box for all planes is 4.5 % slower), one 3-d box each for the
+//   * one 4-d box (x, y, z, f) per 128-bit field-vector plane of the ring (6 boxes
+//     in fp64; a single box for all planes is 4.5 % slower), one 3-d box each for the
 //     scalar planes az and phi^{n+1} (staged with a 16-byte pad on both sides of a row so that
 //     the box is 16-byte granular): 8 copies per plane for an interior tile in fp64;
 //   * the parts of a box beyond the lattice are zero-filled by the TMA unit; the periodic images
@@ -75,27 +75,14 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const TmaMap* map, int c0
       : "memory");
 }
 
-// L2 prefetch of a box (no shared memory involved): the DRAM access of a plane that will be staged
-// NSTAGE + PF iterations from now starts early, so the staging copy itself finds the data in L2
-__device__ __forceinline__ void tma_prefetch_4d(const TmaMap* map, int c0, int c1, int c2, int c3) {
-  asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global [%0, {%1, %2, %3, %4}];" ::"l"(map),
-               "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-               : "memory");
-}
-__device__ __forceinline__ void tma_prefetch_3d(const TmaMap* map, int c0, int c1, int c2) {
-  asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global [%0, {%1, %2, %3}];" ::"l"(map),
-               "r"(c0), "r"(c1), "r"(c2)
-               : "memory");
-}
-
 // staging slot of one source plane: the ring of the tile, all 14 scalars.  Out-of-range parts of
 // the main boxes are zero-filled by the TMA unit; the periodic images land in the w* arrays and
 // the threads on a wrapped column / row read those instead.
-template <typename T, int TX, int TY, bool PADDED = false>
+template <typename T, int TX, int TY>
 struct TmaStage {
   using M = TileMap<TX, TY, 1>;
-  // cells per field plane: padded to a multiple of 128 bytes when every plane is its own box
-  static constexpr int VP = PADDED ? (TileMap<TX, TY, 1>::CELLS + 7) / 8 * 8 : TileMap<TX, TY, 1>::CELLS;
+  // cells per field plane, padded to a multiple of 128 bytes (every plane is its own box)
+  static constexpr int VP = (TileMap<TX, TY, 1>::CELLS + 7) / 8 * 8;
   using V = typename VecOf<T>::type;
   static constexpr int KV = 12 / VecOf<T>::W;          // 128-bit field-vector planes
   static constexpr int PAD = 16 / int(sizeof(T));      // scalars in 16 bytes
@@ -118,20 +105,14 @@ struct TmaStage {
   static constexpr unsigned B_WXY = KV * 16 + 2 * 16;
 };
 
-// ABL != 0 : timing ablation (wrong results on purpose; never selected in production)
-//   1 = memory only: every thread takes its node from the staging slot and the main threads store
-//       14 + 3 scalars derived from it by a few additions; no reconstruction, exchange or closing
-//   1 + 2 = loads only (one store per thread at the end), 1 + 4 = stores only (no TMA traffic)
-// PF > 0 : the producer also prefetches the main boxes of plane j + NSTAGE + PF into L2
-// SPLIT  : the main field-vector box is issued as KV boxes of one field plane each
-template <typename T, int TX, int TY, int MINB, int NSTAGE, int ABL = 0, int PF = 0, bool SPLIT = false>
+template <typename T, int TX, int TY, int MINB, int NSTAGE>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS + 32), MINB)
 k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __restrict__ D,
                      T* __restrict__ Qout, int zchunk) {
   using M = TileMap<TX, TY, 1>;
   using SM = K2FastSmem<T, M::CELLS, M::NMAIN>;
   using XB = ExBuf<T, M::CELLS, M::NMAIN>;
-  using STG = TmaStage<T, TX, TY, SPLIT>;
+  using STG = TmaStage<T, TX, TY>;
   using V = typename VecOf<T>::type;
   constexpr int W = VecOf<T>::W;
   extern __shared__ __align__(128) unsigned char tma_smem_raw[];
@@ -167,22 +148,19 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
     const int xsa_w = xw_l ? P.nx - STG::PAD : 0;              // ... of the 16-byte scalar group
     const int ys_w = yw_b ? P.ny - 1 : 0;                      // source row of the wrapped row
     auto produce = [&](int j, int slot) {
-      if (j > z1 || (ABL & 4)) return;
-      if (PF > 0 && lane >= 16 && lane < 19 && j + PF <= z1) {   // L2 prefetch, main boxes only
-        const int jp = j + PF >= P.nz ? j + PF - P.nz : (j + PF < 0 ? j + PF + P.nz : j + PF);
-        if (lane == 16) tma_prefetch_4d(&maps.vec[0], (gx0 - 1) * W, gy0 - 1, jp, 0);
-        else tma_prefetch_3d(lane == 17 ? &maps.az[0] : &maps.ph[0], gx0 - STG::PAD, gy0 - 1, jp);
-      }
+      if (j > z1) return;
       const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
       STG& st = stg[slot];
       unsigned long long* bar = &full[slot];
       if (lane == 0) mbar_expect_tx(bar, bytes);
       __syncwarp();
-      const int kind = lane / 3, what = lane % 3;              // kind: main, wx, wy, wxy
-      if (SPLIT && lane >= 20 && lane < 20 + STG::KV)
+      // lanes 20 .. 20+KV-1: one box per 128-bit field-vector plane of the whole ring
+      if (lane >= 20 && lane < 20 + STG::KV)
         tma_load_4d(&st.vec[lane - 20][0], &maps.vecf, (gx0 - 1) * W, gy0 - 1, jz, lane - 20, bar);
-      if (SPLIT && lane == 0) return;
-      if (lane >= 12) return;
+      // lanes 1 .. 11: kind = lane / 3 (main, wx, wy, wxy), what = lane % 3 (vectors, az, phi);
+      // lane 0 (the main vector box) is covered by the per-plane boxes above
+      if (lane == 0 || lane >= 12) return;
+      const int kind = lane / 3, what = lane % 3;
       if (kind == 1 && !xw) return;
       if (kind == 2 && !yw) return;
       if (kind == 3 && !(xw && yw)) return;
@@ -190,7 +168,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
       const int y = roww ? ys_w : gy0 - 1;
       if (what == 0) {
         const int x = (colw ? xs_w : gx0 - 1) * W;
-        void* dst = kind == 0 ? (void*)&st.vec[0][0] : kind == 1 ? (void*)&st.vwx[0][0]
+        void* dst = kind == 1 ? (void*)&st.vwx[0][0]
                   : kind == 2 ? (void*)&st.vwy[0][0] : (void*)&st.vwxy[0];
         tma_load_4d(dst, &maps.vec[kind], x, y, jz, 0, bar);
       } else {
@@ -257,9 +235,8 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
                   T (&aA)[6], T (&aB)[6], T (&zA)[3], T (&zB)[3], const T (&uPrev)[3],
                   T (&uCur)[3]) {
     T ownE = 0, ownO = 0, ownQ = 0;
-    T abl[13] = {};
     ph_m = ph_0; ph_0 = ph_p;
-    if (!(ABL & 4)) mbar_wait(&full[slot], parity);    // plane j has landed
+    mbar_wait(&full[slot], parity);                    // plane j has landed
     if (in_ring) {
       T cur[13];
       const unsigned char* sb = reinterpret_cast<const unsigned char*>(&stg[slot]);
@@ -268,11 +245,6 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
         unpack(*reinterpret_cast<const V*>(sb + voff + k * vstride), &cur[k * W]);
       cur[12] = *reinterpret_cast<const T*>(sb + azoff);
       ph_p = *reinterpret_cast<const T*>(sb + phoff);
-      if (ABL & 1) {
-        abl[0] = cur[0] + ph_p;
-#pragma unroll
-        for (int f = 1; f < 13; ++f) abl[f] = cur[f];
-      } else {
       uCur[0] = cur[F_UX]; uCur[1] = cur[F_UY]; uCur[2] = cur[F_UZ];
       SrcFields<T> sf;
       const Coef<T> cf = coef_from13(cur);
@@ -286,27 +258,8 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
           xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
       }
       xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
-      }
     }
     __syncthreads();
-    if (ABL & 1) {
-      if (ABL & 2) {                                   // loads only: keep the values alive
-#pragma unroll
-        for (int f = 0; f < 13; ++f) aA[0] += abl[f];
-        if (is_out && j == z1) D[gx + P.nx * gy + (long long)plane * (j - 1)] = aA[0] + ph_p;
-      } else if (is_out && j - 1 >= z0) {
-        NodeOut<T> out;
-        out.p = abl[0]; out.ux = abl[1]; out.uy = abl[2]; out.uz = abl[3];
-        out.axx = abl[4]; out.ayy = abl[5]; out.azz = abl[6]; out.axy = abl[7];
-        out.axz = abl[8]; out.ayz = abl[9]; out.ax = abl[10]; out.ay = abl[11]; out.az = abl[12];
-        const long long idx = gx + P.nx * gy + (long long)plane * (j - 1);
-        store_out(D, P.N, idx, out);
-        T q[3] = {abl[1] + ph_p, abl[2] + ph_p, abl[3] + ph_p};
-        store_q(Qout, P.N, idx, q);
-      }
-      return;
-    }
-
 
     if (is_out) {
       Red6<T> rE, rO, rQ;

@@ -75,6 +75,13 @@ def test_create_argument_errors(B):
     assert lib.tslb_create(32, 32, 32, C.byref(good(B, mu_l=-1.0)), fake, None, C.byref(h)) == -1
     assert lib.tslb_create(32, 32, 32, C.byref(good(B, bc=(0, 2, 0))), fake, None, C.byref(h)) == -1
     assert lib.tslb_create(32, 32, 32, C.byref(good(B)), fake, None, None) == -1
+    # flags: only the documented validation selectors; a stray bit never selects anything
+    for ok in (0, 1, 2, 4, 8, 16, 8 | 16):
+        assert lib.tslb_create(32, 32, 32, C.byref(good(B, flags=ok)), fake, None, C.byref(h)) == 0
+        lib.tslb_destroy(h)
+    for stray in (32, 1 << 8, 59 << 8, 1 << 16, 1 << 23):
+        assert lib.tslb_create(32, 32, 32, C.byref(good(B, flags=stray)), fake, None,
+                               C.byref(h)) == -1
     assert lib.tslb_step(None, 1) == -1
     lib.tslb_destroy(None)
 

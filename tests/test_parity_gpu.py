@@ -121,61 +121,70 @@ def test_laplace_128_short_fp64(ref, path):
         assert not bad, (n, bad)
 
 
-@pytest.mark.parametrize("flags", [2, 2 | (1 << 8)] + [v << 8 for v in list(range(10)) + list(range(30, 33)) + list(range(36, 41)) + [45, 46, 50, 51, 54, 55, 56]] + [v << 16 for v in range(1, 12)])
-def test_kernel_variants_fp64(ref, flags):
-    """Every tuning variant of the lean periodic kernel (flags bits 8-15) and the wall-capable
-    kernel forced onto a periodic box (TSLB_FLAG_GENERIC) meet the same bar."""
-    cfg, steps = _small_case("ragged_periodic")
-    cfg["shape"] = (40, 37, 70)                     # 3 x 5 tiles of 32 x 8, two z chunks, ragged
-    cfg["phi"] = I.sphere_profile(cfg["shape"], (30.3, 16.1, 19.7), 9.0, 4.0)
-    cfg["u"] = I.noise_u(cfg["shape"], 1e-3, 31)
-    steps = [1, 12]
+def _check_both_precisions(ref, cfg, steps, flags, tag):
     want = run_oracle(ref, cfg, steps)
     for prec, tol, fields in (("f64", TOL64, ("rho", "p", "u", "phi")), ("f32", TOL32, ("u", "phi"))):
         got, _ = run_gpu(cfg, steps, prec, flags)
         for n, g, r in zip(steps, got, want):
             errs, bad = compare(ref, cfg, g, r, tol, fields=fields,
                                 state_tol=1e-9 if prec == "f64" else None)
-            print(f"[flags={flags:#x} {prec}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
-            assert not bad, (flags, prec, n, bad)
+            print(f"[{tag} {prec}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+            assert not bad, (tag, prec, n, bad)
 
 
-@pytest.mark.parametrize("k1v", [0, 12] + list(range(20, 30)) + [35])
-def test_interface_row_kernel_variants(ref, k1v):
-    """Row kernel of the interface update (several nodes per thread, flags bits 16-23): two x
-    tiles in fp32 (128 + 8 columns), three in fp64 (64 + 64 + 8), ragged in y and z."""
+# validation selectors of include/tslb.h: every one forces another CORRECT kernel of the product
+SELECTORS = {"auto": 0, "generic": 2, "k2_cpasync": 4, "k2_tma": 8, "k1_flux": 16,
+             "k2_tma+k1_flux": 8 | 16, "k2_cpasync+k1_flux": 4 | 16}
+
+
+@pytest.mark.parametrize("sel", list(SELECTORS))
+def test_kernel_selectors(ref, sel):
+    """Every selectable kernel meets the same bar on a box of 3 x 5 tiles of 32 x 8, two z
+    chunks, ragged in every direction (nx = 70: the TMA selector falls back to cp.async)."""
+    cfg, _ = _small_case("ragged_periodic")
+    cfg["shape"] = (40, 37, 70)
+    cfg["phi"] = I.sphere_profile(cfg["shape"], (30.3, 16.1, 19.7), 9.0, 4.0)
+    cfg["u"] = I.noise_u(cfg["shape"], 1e-3, 31)
+    _check_both_precisions(ref, cfg, [1, 12], SELECTORS[sel], sel)
+
+
+@pytest.mark.parametrize("sel", ["auto", "k1_flux"])
+def test_interface_kernels_on_wide_rows(ref, sel):
+    """Row kernel of the interface update (several nodes per thread) and its one-node-per-thread
+    fallback: two x tiles in fp32 (128 + 8 columns), three in fp64 (64 + 64 + 8), ragged in y, z."""
     cfg, _ = _small_case("ragged_periodic")
     cfg["shape"] = (36, 19, 136)
     cfg["phi"] = I.sphere_profile(cfg["shape"], (128.3, 9.1, 16.7), 7.0, 4.0)
     cfg["u"] = I.noise_u(cfg["shape"], 1e-3, 41)
-    steps = [1, 10]
-    want = run_oracle(ref, cfg, steps)
-    for prec, tol, fields in (("f64", TOL64, ("rho", "p", "u", "phi")), ("f32", TOL32, ("u", "phi"))):
-        got, _ = run_gpu(cfg, steps, prec, k1v << 16)
-        for n, g, r in zip(steps, got, want):
-            errs, bad = compare(ref, cfg, g, r, tol, fields=fields,
-                                state_tol=1e-9 if prec == "f64" else None)
-            print(f"[k1v={k1v} {prec}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
-            assert not bad, (k1v, prec, n, bad)
+    _check_both_precisions(ref, cfg, [1, 10], SELECTORS[sel], f"wide rows/{sel}")
 
 
-@pytest.mark.parametrize("nx,variant", [(96, 60), (96, 61), (64, 62), (128, 60), (96, 70), (64, 71), (128, 72), (96, 59), (64, 73), (128, 74), (96, 66)])
-def test_tma_staged_kernel(ref, nx, variant):
-    """Stream-collide kernel with TMA bulk staging (flags bits 8-15 = 60, 62; kept as a measured, rejected variant): x tiles that wrap
-    on the left, on the right, on both sides (nx = 32) and not at all; ragged in y and z."""
+def test_odd_row_length_uses_the_flux_kernel(ref):
+    """nx = 37 is not a multiple of the 128-bit vector width: the library itself falls back to
+    the one-node-per-thread interface kernel (flags = 0)."""
+    cfg, steps = _small_case("ragged_periodic")
+    _check_both_precisions(ref, cfg, [1, 8], 0, "nx=37")
+
+
+@pytest.mark.parametrize("nx", [64, 96, 128])
+def test_tma_staged_kernel(ref, nx):
+    """Stream-collide kernel with TMA tensor staging (production in fp64 on deep grids, forced
+    here by TSLB_FLAG_K2_TMA in both precisions): x tiles that wrap on the left, on the right,
+    and not at all; the wrapped row / corner boxes; ragged in y and z, 70 planes = two chunks
+    with a ragged tail."""
     cfg, _ = _small_case("ragged_periodic")
     cfg["shape"] = (70, 19, nx)
     cfg["phi"] = I.sphere_profile(cfg["shape"], (nx - 2.7, 9.1, 30.7), 7.0, 4.0)
     cfg["u"] = I.noise_u(cfg["shape"], 1e-3, 43)
-    steps = [1, 10]
-    want = run_oracle(ref, cfg, steps)
-    for prec, tol, fields in (("f64", TOL64, ("rho", "p", "u", "phi")), ("f32", TOL32, ("u", "phi"))):
-        got, _ = run_gpu(cfg, steps, prec, variant << 8)
-        for n, g, r in zip(steps, got, want):
-            errs, bad = compare(ref, cfg, g, r, tol, fields=fields,
-                                state_tol=1e-9 if prec == "f64" else None)
-            print(f"[nx={nx} v={variant} {prec}] step {n}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
-            assert not bad, (nx, variant, prec, n, bad)
+    _check_both_precisions(ref, cfg, [1, 10], SELECTORS["k2_tma"], f"tma nx={nx}")
+
+
+def test_stray_flag_bits_are_rejected():
+    from paper_2501_00846_b200 import binding as B
+    cfg = I.static_droplet(16, 4.0, seed=2)
+    for flags in (32, 1 << 8, 59 << 8, 1 << 16, 1 << 30):
+        with pytest.raises(B.TslbError):
+            B.Solver(16, 16, 16, cfg["params"], flags=flags)
 
 
 def test_host_api_matches_device_api(ref):
