@@ -69,6 +69,7 @@ tslb::DevParams<T> make_dev(int nx, int ny, int nz, const tslb_params& p, long l
   d.kappa_mu = T(3.0 * p.sigma * p.delta / 2.0);
   d.mob = T(p.mobility);
   d.kappa_ac = T(4.0 * p.mobility / p.delta);
+  d.c2 = T(p.mobility * (6.0 / 216.0));
   d.gx = T(p.body_accel[0]); d.gy = T(p.body_accel[1]); d.gz = T(p.body_accel[2]);
   return d;
 }

@@ -96,6 +96,9 @@ struct DevParams {
   T mu_g, dmu;                // mu = mu_g + phi_c dmu                      (R14)
   T beta4, kappa_mu;          // 4 beta = 48 sigma/delta ; 3 sigma delta/2
   T mob, kappa_ac;            // D ; 4 D/delta
+  T c2;                       // D 6/216 rounded to T: weight of the (1,4,1)^3 Laplacian sums in the
+                              // flux-form interface kernels (the centre weight 1 - 216 c2 is never
+                              // formed: the kernels add an increment of differences to phi)
   T gx, gy, gz;               // body acceleration                          (R20)
 };
 
@@ -284,7 +287,7 @@ __device__ __forceinline__ void load_q(const T* Q, long long N, long long idx, T
 
 // ---- cp.async staging of the next source planes (memory pipeline without registers) ---------
 // The kernel is bound by global-memory latency unless several planes per SM are in flight
-// (profiles/r1_ablation.md), and fp64 has no registers to spare for a deeper prefetch.  Each
+// (profiles/r1_tuning_evidence.md), and fp64 has no registers to spare for a deeper prefetch.  Each
 // thread therefore copies the 14 scalars of ITS OWN node for plane j+NSTAGE straight into a
 // private shared-memory slot (cp.async, no register staging) and picks them up NSTAGE iterations
 // later; only cp.async.wait_group is needed, no block barrier, because nobody else reads the slot.

@@ -171,6 +171,47 @@ __device__ __forceinline__ Red6<T> reduce6(const T (&v)[3][3]) {   // v[cx+1][cy
   return r;
 }
 
+// Source plane of marching index j in [-1, nz]: periodic wrap, or (walls at z = 0 / top, R19) the
+// evenly mirrored plane: -1 -> 0, nz -> nz-1.
+__device__ __forceinline__ int source_plane(int j, int nz, int bcz) {
+  if (j < 0) return bcz ? -1 - j : j + nz;
+  if (j >= nz) return bcz ? 2 * nz - 1 - j : j - nz;
+  return j;
+}
+
+// A source node publishes E, O, Qq of its 8 moving in-plane directions at the receivers' indices
+// and keeps the resting direction in registers.
+// Walls on the marching axis (halfway bounce-back, R19: f_c(x) = fpost_{-c}(x) when x - c lies
+// beyond the wall): a GHOST source plane (j = -1 or nz, loaded from the mirrored plane 0 / nz-1)
+// sends nothing across; every node of the wall plane instead receives ITS OWN populations
+// reversed: the arrival with in-plane direction a and vertical direction cz is
+//   P_own(-a, -cz) = E_own(-a) - cz O_own(-a) + (cz^2 - 1/3) Qq_own(-a),
+// i.e. the fields (E_own(-a), -O_own(-a), Qq_own(-a)) in the node's own receiver slots.  The
+// receiver code is the same in both cases: the ghost plane's cz = +1 combination lands on plane 0,
+// its cz = -1 combination on plane nz-1, and the rest falls on planes that do not exist.
+template <typename T, int TX, int TY, typename XB>
+__device__ __forceinline__ void publish(XB& xb, const SrcFields<T>& sf, bool ghost, bool is_main,
+                                        unsigned need, int rb, T& ownE, T& ownO, T& ownQ) {
+  if (!ghost) {
+    ownE = sf.E[1][1]; ownO = sf.O[1][1]; ownQ = sf.Q[1][1];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) {
+      const int cx = q % 3 - 1, cy = q / 3 - 1;
+      if (cx == 0 && cy == 0) continue;
+      if (need >> dir_slot(cx, cy) & 1u)
+        xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
+    }
+  } else if (is_main) {
+    ownE = sf.E[1][1]; ownO = -sf.O[1][1]; ownQ = sf.Q[1][1];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) {
+      const int cx = q % 3 - 1, cy = q / 3 - 1;
+      if (cx == 0 && cy == 0) continue;
+      xb.put(dir_slot(cx, cy), rb, sf.E[1 - cx][1 - cy], -sf.O[1 - cx][1 - cy], sf.Q[1 - cx][1 - cy]);
+    }
+  }
+}
+
 // cp.async staging NSTAGE >= 1 planes ahead: each thread copies the 14 scalars of ITS OWN node
 // for plane j + NSTAGE straight into a private shared-memory slot (StageBuf, tslb_device.cuh)
 // and picks them up NSTAGE iterations later; only cp.async.wait_group is needed.
@@ -208,7 +249,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   auto stage_issue = [&](int j, int slot) {
     if (in_ring && j <= z1) {
       using V = typename VecOf<T>::type;
-      const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
+      const int jz = source_plane(j, P.nz, P.bcz);
       const int s = col + plane * jz;
       const V* g = reinterpret_cast<const V*>(S);
 #pragma unroll
@@ -246,14 +287,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
       SrcFields<T> sf;
       const Coef<T> cf = coef_from13(cur);
       source_fields(cf, sf);
-      ownE = sf.E[1][1]; ownO = sf.O[1][1]; ownQ = sf.Q[1][1];
-#pragma unroll
-      for (int q = 0; q < 9; ++q) {
-        const int cx = q % 3 - 1, cy = q / 3 - 1;
-        if (cx == 0 && cy == 0) continue;
-        if (need >> dir_slot(cx, cy) & 1u)
-          xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
-      }
+      publish<T, TX, TY>(xb, sf, P.bcz && (j < 0 || j >= P.nz), tid < M::NMAIN, need, rb, ownE, ownO, ownQ);
       xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
     }
     stage_issue(j + NSTAGE, slot);             // refill the slot just consumed
@@ -323,7 +357,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         const T gx_ = fma(T(4), rd[1], rd[0] + rd[2]) * T(3.0 / 216.0);
         const T gy_ = (rs[2] - rs[0]) * T(3.0 / 216.0);
         const T gz_ = fma(T(4), zs[1], zs[0] + zs[2]) * T(3.0 / 216.0);
-        const T lap = fma(T(6.0 / 216.0), sw, T(-6) * ph_0);
+        const T lap = T(6.0 / 216.0) * fma(T(-216), ph_0, sw);   // difference form: 0 on constants
         const NodeOut<T> out = close_node(P, m, ph_0, gx_, gy_, gz_, lap, uPrev[0], uPrev[1], uPrev[2]);
         const long long idx = gx + P.nx * gy + (long long)plane * k;
         store_out(D, P.N, idx, out);

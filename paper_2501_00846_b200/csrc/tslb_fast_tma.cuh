@@ -149,7 +149,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
     const int ys_w = yw_b ? P.ny - 1 : 0;                      // source row of the wrapped row
     auto produce = [&](int j, int slot) {
       if (j > z1) return;
-      const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
+      const int jz = source_plane(j, P.nz, P.bcz);
       STG& st = stg[slot];
       unsigned long long* bar = &full[slot];
       if (lane == 0) mbar_expect_tx(bar, bytes);
@@ -249,14 +249,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
       SrcFields<T> sf;
       const Coef<T> cf = coef_from13(cur);
       source_fields(cf, sf);
-      ownE = sf.E[1][1]; ownO = sf.O[1][1]; ownQ = sf.Q[1][1];
-#pragma unroll
-      for (int q = 0; q < 9; ++q) {
-        const int cx = q % 3 - 1, cy = q / 3 - 1;
-        if (cx == 0 && cy == 0) continue;
-        if (need >> dir_slot(cx, cy) & 1u)
-          xb.put(dir_slot(cx, cy), rb + cy * TX + cx, sf.E[cx + 1][cy + 1], sf.O[cx + 1][cy + 1], sf.Q[cx + 1][cy + 1]);
-      }
+      publish<T, TX, TY>(xb, sf, P.bcz && (j < 0 || j >= P.nz), tid < M::NMAIN, need, rb, ownE, ownO, ownQ);
       xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
     }
     __syncthreads();
@@ -325,7 +318,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
         const T gx_ = fma(T(4), rd[1], rd[0] + rd[2]) * T(3.0 / 216.0);
         const T gy_ = (rs[2] - rs[0]) * T(3.0 / 216.0);
         const T gz_ = fma(T(4), zs[1], zs[0] + zs[2]) * T(3.0 / 216.0);
-        const T lap = fma(T(6.0 / 216.0), sw, T(-6) * ph_0);
+        const T lap = T(6.0 / 216.0) * fma(T(-216), ph_0, sw);   // difference form: 0 on constants
         const NodeOut<T> out = close_node(P, m, ph_0, gx_, gy_, gz_, lap, uPrev[0], uPrev[1], uPrev[2]);
         const long long idx = gx + P.nx * gy + (long long)plane * k;
         store_out(D, P.N, idx, out);

@@ -51,7 +51,7 @@ k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__
   const int plane = P.nx * P.ny;
   const int col = in_ring ? sx + P.nx * sy : 0;
   const T* phi = S + F_PHI * P.N;
-  const T c1 = T(-3.0 / 216.0), c2 = P.mob * T(6.0 / 216.0), c0 = T(1) - T(6) * P.mob;
+  const T c1 = T(-3.0 / 216.0), c2 = P.c2;
 
   auto load = [&](int z, T (&q)[3], T& f) {
     const int jz = z < 0 ? z + P.nz : (z >= P.nz ? z - P.nz : z);
@@ -91,7 +91,7 @@ k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__
 
   int slot = 0;
   auto step = [&](const int k, FluxBuf<T, M::CELLS>& w, T (&rq)[3], T& rf) {
-    T own = 0;
+    T a0 = 0, g0 = 0;
 #pragma unroll
     for (int i = 0; i < 3; ++i) { qa[i] = qb[i]; qb[i] = qc[i]; }
     fa = fb; fb = fc;
@@ -111,9 +111,13 @@ k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__
       const T X = fma(T(4), qb[0], qa[0] + qc[0]);
       const T Y = fma(T(4), qb[1], qa[1] + qc[1]);
       const T Z = qc[2] - qa[2];
-      const T pz = fma(T(4), fb, fa + fc);
+      // phi along z in difference form (see tslb_flux_row.cuh): A carries 6 c2 phi and is only
+      // ever used in differences, g0 is the node's own small part
+      const T d2z = (fa - fb) + (fc - fb);
+      const T pz = fma(T(6), fb, d2z);
       const T A = fma(c1, Z, c2 * pz), Bx = c1 * X, By = c1 * Y;
-      own = T(16) * A;
+      a0 = A;
+      g0 = fma(c1, Z, c2 * d2z);
       const T apx = A + Bx, amx = A - Bx;
       // direction d = (dx,dy): slots 0..7 = (-1,-1) (0,-1) (1,-1) (-1,0) (1,0) (-1,1) (0,1) (1,1)
       w.dv[0][c] = apx + By;            w.dv[1][c] = T(4) * (A + By);
@@ -124,12 +128,15 @@ k_allen_cahn_flux(DevParams<T> P, const T* __restrict__ S, const T* __restrict__
     __syncthreads();
     if (is_out) {
       // the value sent in direction d arrives from the source at -d
-      T s = own;
-      s += (w.dv[0][c + M::W + 1] + w.dv[7][c - M::W - 1])          // (-1,-1) , (1,1)
-         + (w.dv[2][c + M::W - 1] + w.dv[5][c - M::W + 1]);         // (1,-1)  , (-1,1)
-      s += (w.dv[1][c + M::W] + w.dv[6][c - M::W])                  // (0,-1)  , (0,1)
-         + (w.dv[3][c + 1] + w.dv[4][c - 1]);                       // (-1,0)  , (1,0)
-      phin[gx + P.nx * gy + plane * k] = fma(c0, fb, s);
+      // every arrival minus its weight times the own A: a sum of small differences, so that
+      // phi' = phi + 36 g0 + (...) is an increment on top of phi (the 36 A + c0 phi of the plain
+      // flux form cancel symbolically: c0 + 216 c2 = 1)
+      const T a4 = T(4) * a0;
+      T s = ((w.dv[0][c + M::W + 1] - a0) + (w.dv[7][c - M::W - 1] - a0))          // (-1,-1) , (1,1)
+          + ((w.dv[2][c + M::W - 1] - a0) + (w.dv[5][c - M::W + 1] - a0));         // (1,-1)  , (-1,1)
+      s += ((w.dv[1][c + M::W] - a4) + (w.dv[6][c - M::W] - a4))                   // (0,-1)  , (0,1)
+         + ((w.dv[3][c + 1] - a4) + (w.dv[4][c - 1] - a4));                        // (-1,0)  , (1,0)
+      phin[gx + P.nx * gy + plane * k] = fb + fma(T(36), g0, s);
     }
   };
   for (int k = z0; k < z1; k += 2) {

@@ -45,8 +45,9 @@ template <typename T, int TY, int NSTAGE>
 struct RowSmem {
   using vec = typename RowVec<T>::vec;
   static constexpr int ROWS = TY + 2;
-  vec um[2][ROWS][32];              // (R - S) of the V nodes of a thread, double buffered over k
-  vec up[2][ROWS][32];              // (R + S)
+  vec um[2][ROWS][32];              // (Dx - S) of the V nodes of a thread, double buffered over k
+  vec up[2][ROWS][32];              // (Dx + S)
+  vec aa[2][ROWS][32];              // A itself (the rows above and below difference it with theirs)
   T xh[2][ROWS][2][2];              // [k & 1][row][side]{A -+ Bx, By} of the columns beside the tile
   vec stage[NSTAGE][4][ROWS][32];   // Qx, Qy, Qz, phi of the thread's nodes, one slot per plane
   T xstage[NSTAGE][4][2 * ROWS];    // the same for the single-node columns of the extra warp
@@ -81,7 +82,7 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
   const int z1 = min(P.nz, z0 + zchunk);
   const int plane = P.nx * P.ny;
   const T* phi = S + F_PHI * P.N;
-  const T c1 = T(-3.0 / 216.0), c2 = P.mob * T(6.0 / 216.0), c0 = T(1) - T(6) * P.mob;
+  const T c1 = T(-3.0 / 216.0), c2 = P.c2;
 
   // row of this thread: row warps own row `warp`; lane h of the extra warp owns row h / 2
   const int row = xhalo ? (lane >> 1) : warp;
@@ -100,9 +101,33 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
   const bool is_out = !xhalo && active && row >= 1 && row <= TY && gy < P.ny;
   const int col = active ? sx + P.nx * sy : 0;
 
+  // Walls on the marching axis (R19): the ghost plane j = -1 / nz is the mirrored plane m = 0 /
+  // nz-1 with phi even, the advective flux phi u odd in every component (no slip) and the
+  // sharpening flux odd in its wall-normal component only (neutral wetting).  In terms of the
+  // stored total flux Q = phi u + kappa phi (1-phi) n:
+  //   Qx(ghost) = Qx(m) - 2 phi(m) ux(m),  Qy likewise,  Qz(ghost) = -Qz(m),  phi(ghost) = phi(m),
+  // so the two ghost iterations of a column also read u of the wall plane.
+  auto zsrc = [&](int j) {
+    if (j < 0) return P.bcz ? -1 - j : j + P.nz;
+    if (j >= P.nz) return P.bcz ? 2 * P.nz - 1 - j : j - P.nz;
+    return j;
+  };
+  auto ghostify = [&](int j, T (&qx)[V], T (&qy)[V], T (&qz)[V], const T (&f)[V]) {
+    if (!(P.bcz && (j < 0 || j >= P.nz)) || !active) return;
+    const long long s = col + (long long)plane * zsrc(j);
+#pragma unroll
+    for (int i = 0; i < V; ++i) {
+      if (xhalo && i > 0) break;
+      T ux, uy, uz;
+      load_u(S, P.N, s + i, ux, uy, uz);
+      qx[i] = fma(T(-2) * f[i], ux, qx[i]);
+      qy[i] = fma(T(-2) * f[i], uy, qy[i]);
+      qz[i] = -qz[i];
+    }
+  };
   auto issue = [&](int j, int slot) {              // one commit group per plane, possibly empty
     if (active && j <= z1) {
-      const int jz = j < 0 ? j + P.nz : (j >= P.nz ? j - P.nz : j);
+      const int jz = zsrc(j);
       const long long s = col + (long long)plane * jz;
       if (xhalo) {
         cp_async_small(&sm.xstage[slot][0][lane], Q + s);
@@ -120,8 +145,8 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
   };
 
   // running accumulators (see zsum141) and the two older planes of Qz
-  T xa[V] = {}, xb[V] = {}, ya[V] = {}, yb[V] = {}, pa[V] = {}, pb[V] = {}, zm[V] = {}, z0v[V] = {};
-  T A[V], Bx[V], By[V], fb[V];
+  T xa[V] = {}, xb[V] = {}, ya[V] = {}, yb[V] = {}, pm[V] = {}, pb[V] = {}, zm[V] = {}, z0v[V] = {};
+  T A[V], Bx[V], By[V], fb[V], g0[V];
 
   // receive one plane of the own nodes: afterwards A, Bx, By, fb describe the plane before it
   auto receive = [&](const T (&qx)[V], const T (&qy)[V], const T (&qz)[V], const T (&f)[V]) {
@@ -130,15 +155,19 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
       fb[i] = pb[i];
       const T X = zsum141(qx[i], xa[i], xb[i]);
       const T Y = zsum141(qy[i], ya[i], yb[i]);
-      const T pz = zsum141(f[i], pa[i], pb[i]);
+      // phi along z in DIFFERENCE form: d2z = phi(k-1) - 2 phi(k) + phi(k+1), pz = 6 phi(k) + d2z
+      const T d2z = (pm[i] - pb[i]) + (f[i] - pb[i]);
+      const T pz = fma(T(6), pb[i], d2z);
+      pm[i] = pb[i]; pb[i] = f[i];
       const T Z = qz[i] - zm[i];
       zm[i] = z0v[i]; z0v[i] = qz[i];
-      A[i] = fma(c1, Z, c2 * pz);
+      A[i] = fma(c1, Z, c2 * pz);          // carries 6 c2 phi: only ever used in differences
+      g0[i] = fma(c1, Z, c2 * d2z);        // the same without it: the node's own small part
       Bx[i] = c1 * X;
       By[i] = c1 * Y;
     }
   };
-  auto take = [&](int slot) {
+  auto take = [&](int slot, int j) {
     T qx[V] = {}, qy[V] = {}, qz[V] = {}, f[V] = {};
     if (active) {
       if (xhalo) {
@@ -151,6 +180,7 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
         RV::get(sm.stage[slot][3][row][lane], f);
       }
     }
+    ghostify(j, qx, qy, qz, f);
     receive(qx, qy, qz, f);
   };
 
@@ -162,11 +192,11 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
   if (xhalo) {                                      // plane z0-1 of the extra warp, before the loop
     T qx[V] = {}, qy[V] = {}, qz[V] = {}, f[V] = {};
     if (active) {
-      const int jz = z0 - 1 < 0 ? z0 - 1 + P.nz : z0 - 1;
-      const long long s = col + (long long)plane * jz;
+      const long long s = col + (long long)plane * zsrc(z0 - 1);
       qx[0] = __ldg(Q + s); qy[0] = __ldg(Q + P.N + s); qz[0] = __ldg(Q + 2 * P.N + s);
       f[0] = __ldg(phi + s);
     }
+    ghostify(z0 - 1, qx, qy, qz, f);
     receive(qx, qy, qz, f);
   }
 #pragma unroll
@@ -175,11 +205,11 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
   for (int j = z0 - 1; j <= z1; ++j) {
     const int k = j - 1;
     cp_async_wait<NSTAGE - 1>();                    // the group of plane j + lead has landed
-    take(slot);
+    take(slot, j + lead);
     issue(j + lead + NSTAGE, slot);
     slot = (slot + 1 == NSTAGE) ? 0 : slot + 1;
 
-    T R[V], Sy[V];
+    T Dx[V], Sy[V];
     if (xhalo) {
       // combinations of plane j (= k + 1) for the row warps' next iteration
       if (active) {
@@ -202,24 +232,37 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
         const T right = i == V - 1 ? rp : A[i + 1] + Bx[i + 1];
         const T bl = i == 0 ? lby : By[i - 1];
         const T br = i == V - 1 ? rby : By[i + 1];
-        R[i] = fma(T(4), A[i], left + right);
+        Dx[i] = (left - A[i]) + (right - A[i]);      // R = 6 A + Dx is never formed
         Sy[i] = fma(T(4), By[i], bl + br);
       }
       if (active) {
         T d[V], s[V];
 #pragma unroll
-        for (int i = 0; i < V; ++i) { d[i] = R[i] - Sy[i]; s[i] = R[i] + Sy[i]; }
+        for (int i = 0; i < V; ++i) { d[i] = Dx[i] - Sy[i]; s[i] = Dx[i] + Sy[i]; }
         if (row <= TY - 1) sm.um[k & 1][row][lane] = RV::make(d);      // read by row + 1
         if (row >= 2) sm.up[k & 1][row][lane] = RV::make(s);           // read by row - 1
+        sm.aa[k & 1][row][lane] = RV::make(A);                         // read by rows +- 1
       }
     }
     __syncthreads();
     if (is_out && k >= z0) {
-      T lo[V], hi[V], o[V];
+      // phi' = c0 phi + sum_y w_y (R -+ S)(y) with R = 6 A + Dx, A = g0 + 6 c2 phi and
+      // c0 + 216 c2 = 1 becomes, with every O(phi) term cancelled symbolically,
+      //   phi' = phi + 36 g0 + 6 [(A(y-1) - A) + (A(y+1) - A)] + 4 Dx + (Dx - S)(y-1) + (Dx + S)(y+1):
+      // an increment of small terms on top of phi, as in the oracle's phi - div Q + D lap(phi)
+      // with the Laplacian as a sum of differences; the flux form's own c0 phi + 0.3 phi-sized
+      // partial sums cost ~10x more rounding noise in phi per step.
+      T lo[V], hi[V], alo[V], ahi[V], o[V];
       RV::get(sm.um[k & 1][row - 1][lane], lo);
       RV::get(sm.up[k & 1][row + 1][lane], hi);
+      RV::get(sm.aa[k & 1][row - 1][lane], alo);
+      RV::get(sm.aa[k & 1][row + 1][lane], ahi);
 #pragma unroll
-      for (int i = 0; i < V; ++i) o[i] = fma(c0, fb[i], fma(T(4), R[i], lo[i] + hi[i]));
+      for (int i = 0; i < V; ++i) {
+        const T ty = (alo[i] - A[i]) + (ahi[i] - A[i]);
+        const T inc = fma(T(36), g0[i], fma(T(6), ty, fma(T(4), Dx[i], lo[i] + hi[i])));
+        o[i] = fb[i] + inc;
+      }
       *reinterpret_cast<vec*>(phin + (sx + P.nx * gy + (long long)plane * k)) = RV::make(o);
     }
   }

@@ -231,14 +231,19 @@ template <typename T>
 int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
                       long long* launches, const Marker& mk, int flags, TmaCache* tc = nullptr) {
   const bool walls = P.bcx || P.bcy || P.bcz;
-  const bool generic = walls || (flags & SEL_GENERIC);
+  // The lean pair serves periodic tile axes (x, y); walls on the MARCHING axis z (configs[2]:
+  // no-slip floor and lid) cost it two ghost planes per column (bounce-back in publish(), ghost
+  // flux in the row kernel).  Walls on x or y, or rows that the row kernel cannot vectorise on a
+  // box with walls, run the wall-capable pair.
+  const bool row_ok = P.nx % RowVec<T>::V == 0;
+  const bool generic = P.bcx || P.bcy || (P.bcz && !row_ok) || (flags & SEL_GENERIC);
   cudaError_t e;
   // ---- K1
   if (generic) {
     // wall-capable: normals recomputed on a ring of depth 2 (the two parts of the flux mirror
     // differently at a wall, so the flux form cannot serve walls)
     e = walls ? launch_k1w<T, true>(P, S, D, stream) : launch_k1w<T, false>(P, S, D, stream);
-  } else if (P.nx % RowVec<T>::V == 0 && !(flags & SEL_K1_FLUX)) {
+  } else if (row_ok && (P.bcz || !(flags & SEL_K1_FLUX))) {
     e = launch_k1_row<T>(P, S, Q, D, stream);
   } else {
     e = launch_k1_flux<T>(P, S, Q, D, stream);

@@ -32,20 +32,21 @@ template <typename T>
 __device__ __forceinline__ void grad_lap(const DevParams<T>& P, const T* __restrict__ phi, int ix,
                                          int iy, int iz, T& gx, T& gy, T& gz, T& lap) {
   T sx = 0, sy = 0, sz = 0, sw = 0;
+  const T p0 = phi[ix + (long long)P.nx * (iy + (long long)P.ny * iz)];
 #pragma unroll
   for (int i = 0; i < 27; ++i) {
     const int cx = i % 3 - 1, cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
     int kx, ky, kz;
     T v = phi[nbr(P, ix, iy, iz, cx, cy, cz, kx, ky, kz)];
     T w = w1<T>(cx) * w1<T>(cy) * w1<T>(cz);
-    sw = fma(w, v, sw);
+    sw = fma(w, v - p0, sw);                      // differences first: exactly 0 on constants
     if (cx) sx = fma(w * T(cx), v, sx);
     if (cy) sy = fma(w * T(cy), v, sy);
     if (cz) sz = fma(w * T(cz), v, sz);
   }
   gx = T(3) * sx; gy = T(3) * sy; gz = T(3) * sz;
-  // (2/cs^2) sum_{i!=0} w_i (phi_i - phi_0) = 6 (sum_i w_i phi_i - phi_0)
-  lap = T(6) * (sw - phi[ix + (long long)P.nx * (iy + (long long)P.ny * iz)]);
+  // (2/cs^2) sum_{i!=0} w_i (phi_i - phi_0) = 6 sum_i w_i (phi_i - phi_0)
+  lap = T(6) * sw;
 }
 
 // ---- stage K4a: sharpening flux  Qs = phi (1 - phi) grad(phi)/sqrt(|grad(phi)|^2 + eps^2)  (R13)
@@ -79,6 +80,7 @@ __global__ void __launch_bounds__(256) k_allen_cahn_naive(DevParams<T> P, long l
   node_coords(P, idx, ix, iy, iz);
   const T* phi = S + F_PHI * P.N;
   T div = 0, sw = 0;
+  const T p0 = phi[idx];
 #pragma unroll
   for (int i = 0; i < 27; ++i) {
     const int cx = i % 3 - 1, cy = (i / 3) % 3 - 1, cz = i / 9 - 1;
@@ -86,7 +88,7 @@ __global__ void __launch_bounds__(256) k_allen_cahn_naive(DevParams<T> P, long l
     long long j = nbr(P, ix, iy, iz, cx, cy, cz, kx, ky, kz);
     T w = w1<T>(cx) * w1<T>(cy) * w1<T>(cz);
     T pj = phi[j];
-    sw = fma(w, pj, sw);
+    sw = fma(w, pj - p0, sw);                     // differences first: exactly 0 on constants
     if (cx || cy || cz) {
       // velocity-like ghosts: every component flips once per wall crossed (R19)
       T s0 = ((kx + ky + kz) & 1) ? T(-1) : T(1);
@@ -98,8 +100,7 @@ __global__ void __launch_bounds__(256) k_allen_cahn_naive(DevParams<T> P, long l
       div = fma(w, fl, div);
     }
   }
-  T p0 = phi[idx];
-  phin[idx] = p0 - T(3) * div + P.mob * T(6) * (sw - p0);
+  phin[idx] = p0 - T(3) * div + P.mob * T(6) * sw;
 }
 
 // ---- stage K3+K1+K2: pull-stream with per-source reconstruction, moments, forces, closing

@@ -226,8 +226,8 @@ k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ 
     }
     // z-combinations of phi^{n+1} for the output plane k = j-1 (Eq. 18-19 are separable)
     if (in_ring) {
-      sm.pz[c] = T(1.0 / 6.0) * (ph_m + ph_p) + T(2.0 / 3.0) * ph_0;
-      sm.dz[c] = T(1.0 / 6.0) * (ph_p - ph_m);
+      sm.pz[c] = fma(T(4), ph_0, ph_m + ph_p);     // integer weights (1,4,1); 1/216 deferred
+      sm.dz[c] = ph_p - ph_m;
     }
     __syncthreads();
 
@@ -240,15 +240,17 @@ k_stream_collide_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ 
 #pragma unroll
         for (int q = 0; q < 9; ++q) {
           const int cx = q % 3 - 1, cy = q / 3 - 1;
-          const T w = w1<T>(cx) * w1<T>(cy);
+          const T w = T((cx ? 1 : 4) * (cy ? 1 : 4));
           const T a = sm.pz[c + cy * M::W + cx], b = sm.dz[c + cy * M::W + cx];
           sw_ = fma(w, a, sw_);
           sz_ = fma(w, b, sz_);
           if (cx) sx_ = fma(w * T(cx), a, sx_);
           if (cy) sy_ = fma(w * T(cy), a, sy_);
         }
-        const T lap = T(6) * (sw_ - ph_0);
-        NodeOut<T> o = close_node(P, mom[0], ph_0, T(3) * sx_, T(3) * sy_, T(3) * sz_, lap,
+        // Laplacian in difference form (exactly 0 on constants, like the oracle's Eq. 19)
+        const T lap = T(6.0 / 216.0) * fma(T(-216), ph_0, sw_);
+        const T g3 = T(3.0 / 216.0);
+        NodeOut<T> o = close_node(P, mom[0], ph_0, g3 * sx_, g3 * sy_, g3 * sz_, lap,
                                   uo[0][0], uo[0][1], uo[0][2]);
         const long long d = gx + (long long)P.nx * gy + plane * k;
         store_out(D, P.N, d, o);
@@ -401,7 +403,7 @@ k_allen_cahn_tiled(DevParams<T> P, const T* __restrict__ S, T* __restrict__ phin
       T div = T(16) * zz1;
       div += (r.dv[0][c + M::W + 1] + r.dv[7][c - M::W - 1]) + (r.dv[2][c + M::W - 1] + r.dv[5][c - M::W + 1]);
       div += (r.dv[1][c + M::W] + r.dv[6][c - M::W]) + (r.dv[3][c + 1] + r.dv[4][c - 1]);
-      const T lap = fma(T(6.0 / 216.0), sw2, T(-6) * ph2);
+      const T lap = T(6.0 / 216.0) * fma(T(-216), ph2, sw2);   // difference form: 0 on constants
       phin[gx + P.nx * gy + plane * k] = ph2 - T(3.0 / 216.0) * div + P.mob * lap;
     }
     sw2 = sw1; sw1 = sw0; ph2 = ph1; ph1 = f0; zz1 = zz0;

@@ -179,6 +179,20 @@ def test_tma_staged_kernel(ref, nx):
     _check_both_precisions(ref, cfg, [1, 10], SELECTORS["k2_tma"], f"tma nx={nx}")
 
 
+@pytest.mark.parametrize("sel", ["auto", "k2_tma", "k2_cpasync", "generic"])
+def test_z_walls_on_the_lean_pair(ref, sel):
+    """Walls on the marching axis (configs[2]: no-slip floor and lid, periodic sides) run the lean
+    periodic pair with bounce-back ghost planes; the wall-capable pair is the cross-check.  Gas
+    bubble touching the floor, a liquid film... two tiles in x, three in y, 70 planes = chunks
+    with a ragged tail, gravity on."""
+    shape = (70, 19, 64)                                         # (nz, ny, nx)
+    prm = I.base_params(bc=(0, 0, 1), body_accel=(1e-6, 0.0, -2e-5))
+    phi = 1.0 - I.sphere_profile(shape, (20.3, 9.1, 4.6), 7.0, 4.0, prm["bc"])     # at the floor
+    phi -= I.sphere_profile(shape, (50.2, 5.7, 66.1), 6.0, 4.0, prm["bc"])          # at the lid
+    cfg = dict(name="z_walls", shape=shape, params=prm, phi=phi, u=I.noise_u(shape, 1e-3, 47))
+    _check_both_precisions(ref, cfg, [1, 2, 14], SELECTORS[sel], f"z walls/{sel}")
+
+
 def test_stray_flag_bits_are_rejected():
     from paper_2501_00846_b200 import binding as B
     cfg = I.static_droplet(16, 4.0, seed=2)
