@@ -101,7 +101,7 @@ int tslb_get_state(tslb_handle *h, void *pstar, void *u, void *A, void *a, void 
  * Fig. 4) and BASELINE.json's checks (sum(phi) conserved; Laplace's law
  * Delta p R/(2 sigma) on configs[1]), so that no whole field has to be read back.
  * out = TSLB_NDIAG doubles (fp64 accumulation in both precisions), indexed by TSLB_D_*:
- *   SUM_PHI, SUM_PSTAR, MAX_U (max |u|), SUM_PHI_X/Y/Z (sum phi * node index: centre of mass of
+ *   SUM_PHI, SUM_PSTAR, MAX_U (max |u|; NaN if any velocity is NaN), SUM_PHI_X/Y/Z (sum phi * node index: centre of mass of
  *   the liquid = SUM_PHI_X / SUM_PHI on a non-periodic axis), SUM_PHI_UX/UY/UZ (its momentum per
  *   unit liquid density), SUM_UX/UY/UZ (so the light phase's is sum(u) - sum(phi u)),
  *   SUM_P_IN / N_IN: sum and count of p = p* rho cs^2 over nodes with phi > 0.99,

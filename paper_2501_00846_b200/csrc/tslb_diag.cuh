@@ -115,7 +115,13 @@ k_diag_final(const double* __restrict__ partial, long long rows, double* __restr
     }
     __syncthreads();
   }
-  if (threadIdx.x < NDIAG) out[threadIdx.x] = red[0][threadIdx.x];
+  // fmax drops NaNs: a non-finite velocity field must not read as max|u| = 0
+  if (threadIdx.x < NDIAG) {
+    double v = red[0][threadIdx.x];
+    const double su = red[0][9] + red[0][10] + red[0][11];
+    if (threadIdx.x == 2 && su != su) v = su;
+    out[threadIdx.x] = v;
+  }
 }
 
 }  // namespace tslb

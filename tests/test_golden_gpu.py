@@ -53,6 +53,18 @@ def _errors(g, gold, cp, idx):
 @pytest.mark.parametrize("case", list(CASES))
 @pytest.mark.parametrize("precision", ["f64", "f32"])
 def test_against_golden(case, precision):
+    _replay(case, precision, 0)
+
+
+@pytest.mark.parametrize("flags", [1, 2, 16], ids=["naive", "generic", "k1_flux"])
+def test_laplace_horizon_on_every_path(flags):
+    """configs[1]'s own horizon (R = 12, 2000 steps) through the other kernels of the product:
+    the one-thread-per-node path, the wall-capable pair and the one-node interface kernel meet the
+    same twin-based bar as the production pair ("the round-1 anomaly")."""
+    _replay("laplace128_R12", "f64", flags)
+
+
+def _replay(case, precision, flags):
     path = os.path.join(HERE, case + ".npz")
     if not os.path.exists(path):
         pytest.skip(f"{path} not generated")
@@ -66,7 +78,7 @@ def test_against_golden(case, precision):
         pytest.skip("lattice does not fit on this GPU")
     nz, ny, nx = cfg["shape"]
     idx = torch.as_tensor(gold["sample_index"], device="cuda")
-    s = B.Solver(nx, ny, nz, cfg["params"], precision=precision)
+    s = B.Solver(nx, ny, nz, cfg["params"], precision=precision, flags=flags)
     s.init(cfg["phi"], cfg["u"])
     done = 0
     tol = 1e-10 if precision == "f64" else 1e-4
@@ -81,7 +93,7 @@ def test_against_golden(case, precision):
         st = s.get_state()
         sum_phi = float(g["phi"].double().sum())
         sum_ps = float(st["pstar"].double().sum())
-        print(f"[{case} {precision}] step {cp}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items())
+        print(f"[{case} {precision}{' flags=%d' % flags if flags else ''}] step {cp}: " + " ".join(f"{k}={v:.2e}" for k, v in errs.items())
               + f" | sum(phi) rel diff {sum_phi / gold[f'diag_{cp}'][0] - 1:.1e}"
               + f" sum(p*) {sum_ps:.1e} (oracle {gold[f'diag_{cp}'][1]:.1e})")
         names = ("rho", "p", "u", "phi")
