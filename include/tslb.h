@@ -21,7 +21,7 @@
  *                      delta/mobility, sigma < 0, unknown enum, axis shorter than the stencil)
  *   TSLB_EWORKSPACE(-2) workspace NULL, too small or not 256-byte aligned
  *   TSLB_ECUDA    (-3) a CUDA call failed (text holds cudaGetErrorString)
- *   TSLB_ESTATE   (-4) tslb_step / tslb_get before tslb_init
+ *   TSLB_ESTATE   (-4) tslb_step / tslb_get before tslb_init (or tslb_set_state)
  */
 #ifndef TSLB_H
 #define TSLB_H
@@ -95,6 +95,15 @@ int tslb_get(tslb_handle *h, void *rho, void *p, void *u, void *phi);
 /* Full internal state (debug / parity of the unexposed fields): p*[N], u[3][N], a2_neq[6][N] in
  * the order xx,yy,zz,xy,xz,yz, a[3][N], phi[N]; DEVICE arrays, NULL skips. */
 int tslb_get_state(tslb_handle *h, void *pstar, void *u, void *A, void *a, void *phi);
+
+/* Restart / resume: the inverse of tslb_get_state.  DEVICE arrays in the handle's precision,
+ * same shapes and order (A holds what tslb_get_state returns: (1 - omega(phi)) a2_neq); all
+ * five are required.  Replaces the whole state, so it may be called instead of tslb_init; the
+ * arrays are not retained.  get_state -> set_state -> step continues a run to rounding (the
+ * flux of Eq. 20 handed between the two kernels of a step is rebuilt from phi and u with another
+ * summation order), not bit for bit. */
+int tslb_set_state(tslb_handle *h, const void *pstar, const void *u, const void *A, const void *a,
+                   const void *phi);
 
 /* On-device diagnostics: box reductions of the current state, the
  * quantities behind the paper's validation plots (centre-of-mass velocity of a rising bubble,

@@ -20,7 +20,7 @@ DIAG_NAMES = ("sum_phi", "sum_pstar", "max_u", "sum_phi_x", "sum_phi_y", "sum_ph
               "sum_p_in", "n_in", "sum_p_out", "n_out")
 
 SYMBOLS = ("tslb_workspace_bytes", "tslb_create", "tslb_init", "tslb_step", "tslb_get",
-           "tslb_get_state", "tslb_init_host", "tslb_get_host", "tslb_step_timed",
+           "tslb_get_state", "tslb_set_state", "tslb_init_host", "tslb_get_host", "tslb_step_timed",
            "tslb_launch_count", "tslb_diag", "tslb_diag_host", "tslb_diag_static", "tslb_fma_peak",
            "tslb_destroy", "tslb_last_error")
 
@@ -65,6 +65,7 @@ def load():
     lib.tslb_step.argtypes = [vp, C.c_int]
     lib.tslb_get.argtypes = [vp, vp, vp, vp, vp]
     lib.tslb_get_state.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.tslb_set_state.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.tslb_init_host.argtypes = [vp, vp, vp]
     lib.tslb_get_host.argtypes = [vp, vp, vp, vp, vp]
     lib.tslb_step_timed.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
@@ -188,6 +189,15 @@ class Solver:
         self._call("tslb_get_state", out["pstar"].data_ptr(), out["u"].data_ptr(),
                    out["A"].data_ptr(), out["a"].data_ptr(), out["phi"].data_ptr())
         return out
+
+    def set_state(self, state):
+        """tslb_set_state from a dict as get_state returns it (restart / resume)."""
+        t = {"pstar": self._dev(state["pstar"], self.shape), "u": self._dev(state["u"], (3,) + self.shape),
+             "A": self._dev(state["A"], (6,) + self.shape), "a": self._dev(state["a"], (3,) + self.shape),
+             "phi": self._dev(state["phi"], self.shape)}
+        self._call("tslb_set_state", t["pstar"].data_ptr(), t["u"].data_ptr(), t["A"].data_ptr(),
+                   t["a"].data_ptr(), t["phi"].data_ptr())
+        self.stream.synchronize()          # the arrays may be temporaries
 
     def diag(self):
         """tslb_diag_host: dict of the TSLB_D_* box reductions (synchronises the stream)."""

@@ -284,6 +284,28 @@ int tslb_get_state(tslb_handle* h, void* pstar, void* u, void* A, void* a, void*
   return TSLB_OK;
 }
 
+int tslb_set_state(tslb_handle* h, const void* pstar, const void* u, const void* A, const void* a,
+                   const void* phi) {
+  if (!h || !pstar || !u || !A || !a || !phi) return fail(TSLB_EINVAL, "tslb_set_state: NULL argument");
+  unsigned blocks = unsigned((h->nodes + 255) / 256);
+  h->cur = 0;
+  if (h->prm.precision == TSLB_F64) {
+    auto P = make_dev<double>(h->nx, h->ny, h->nz, h->prm, h->stride);
+    tslb::k_set_state<double><<<blocks, 256, 0, h->stream>>>(
+        P, h->nodes, (const double*)pstar, (const double*)u, (const double*)A, (const double*)a,
+        (const double*)phi, reinterpret_cast<double*>(h->buf[0]), reinterpret_cast<double*>(h->scratch));
+  } else {
+    auto P = make_dev<float>(h->nx, h->ny, h->nz, h->prm, h->stride);
+    tslb::k_set_state<float><<<blocks, 256, 0, h->stream>>>(
+        P, h->nodes, (const float*)pstar, (const float*)u, (const float*)A, (const float*)a,
+        (const float*)phi, reinterpret_cast<float*>(h->buf[0]), reinterpret_cast<float*>(h->scratch));
+  }
+  h->launches += 1;
+  CUDA_TRY(cudaGetLastError());
+  h->inited = true;
+  return TSLB_OK;
+}
+
 // partial sums into `rows` (device scratch of diag_rows(nodes) rows), result into `out` (device)
 static int diag_launch(tslb_handle* h, double* rows, double* out) {
   const unsigned blocks = unsigned(tslb::diag_rows(h->nodes));

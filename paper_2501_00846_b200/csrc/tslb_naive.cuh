@@ -223,6 +223,34 @@ __global__ void __launch_bounds__(256) k_get(DevParams<T> P, long long nodes,
 }  // namespace tslb
 
 namespace tslb {
+// ---- tslb_set_state: the inverse of tslb_get_state (restart / resume).  The flux Q of Eq. 20 that
+// the periodic interface kernel expects is rebuilt from phi and u as in tslb_init.
+template <typename T>
+__global__ void __launch_bounds__(256) k_set_state(DevParams<T> P, long long nodes,
+                                                   const T* __restrict__ pstar,
+                                                   const T* __restrict__ u, const T* __restrict__ A,
+                                                   const T* __restrict__ a,
+                                                   const T* __restrict__ phi, T* __restrict__ D,
+                                                   T* __restrict__ Q) {
+  long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (idx >= nodes) return;
+  int ix, iy, iz;
+  node_coords(P, idx, ix, iy, iz);
+  T m[13];
+  m[F_P] = pstar[idx];
+  for (int k = 0; k < 3; ++k) m[F_UX + k] = u[k * nodes + idx];
+  for (int k = 0; k < 6; ++k) m[F_AXX + k] = A[k * nodes + idx];
+  for (int k = 0; k < 3; ++k) m[F_AX + k] = a[k * nodes + idx];
+  store13(D, P.N, idx, m);
+  const T ph = phi[idx];
+  D[F_PHI * P.N + idx] = ph;
+  T gx, gy, gz, lap;
+  grad_lap(P, phi, ix, iy, iz, gx, gy, gz, lap);
+  T q[3];
+  flux_q(P, ph, gx, gy, gz, m[F_UX], m[F_UY], m[F_UZ], q);
+  store_q(Q, P.N, idx, q);
+}
+
 // ---- tslb_get_state: de-interleave the stored fields into plain planes (NULL = skip)
 template <typename T>
 __global__ void __launch_bounds__(256) k_get_state(DevParams<T> P, long long nodes,
