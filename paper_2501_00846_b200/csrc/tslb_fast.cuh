@@ -148,6 +148,68 @@ __device__ __forceinline__ void source_fields(const Coef<T>& c, SrcFields<T>& s)
   }
 }
 
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) {      // a - b, one rounding
+  return __ffma2_rn(b, make_float2(-1.f, -1.f), a);
+}
+__device__ __forceinline__ float2 fma4(float2 v, float2 r) {      // 4 v + r
+  return __ffma2_rn(make_float2(4.f, 4.f), v, r);
+}
+
+// fp32: the E and the O polynomial have the same shape (O's lower-order rows are E's with some
+// coefficients zero), so they are evaluated as the two lanes of packed fp32x2 instructions; a lane
+// that has no term there multiplies by 0 (fma(0, x, m) = m exactly), so every component is rounded
+// exactly as in the scalar sequence above.
+__device__ __forceinline__ void source_fields(const Coef<float>& c, SrcFields<float>& s) {
+  const float k = float(1.0 / 216.0);
+  auto f2 = [](float a, float b) { return make_float2(a, b); };
+  float2 A0[3], A1[3], A2[3];                     // lanes: (E's a_n(cx), O's b_n(cx))
+  {
+    const float2 base = __fmul2_rn(f2(k, 3.f * k), f2(c.c0, c.c1z));
+    const float2 q = f2(c.xx, c.xxz), l = f2(c.c1x, c.xz);
+    A0[1] = __ffma2_rn(f2(-1.5f * k, -4.5f * k), q, base);
+    const float2 t = __ffma2_rn(f2(3.f * k, 9.f * k), q, base);
+    A0[0] = __ffma2_rn(f2(-3.f * k, -9.f * k), l, t);
+    A0[2] = __ffma2_rn(f2(3.f * k, 9.f * k), l, t);
+  }
+  {
+    const float2 m1 = __fmul2_rn(f2(3.f * k, 9.f * k), f2(c.c1y, c.yz));
+    const float2 q = f2(c.xxy, 0.f), l = f2(c.xy, c.xyz);
+    A1[1] = __ffma2_rn(f2(-4.5f * k, 0.f), q, m1);
+    const float2 t1 = __ffma2_rn(f2(9.f * k, 0.f), q, m1);
+    A1[0] = __ffma2_rn(f2(-9.f * k, -27.f * k), l, t1);
+    A1[2] = __ffma2_rn(f2(9.f * k, 27.f * k), l, t1);
+  }
+  {
+    A2[1] = __fmul2_rn(f2(4.5f * k, 13.5f * k), f2(c.yy, c.yyz));
+    const float2 q = f2(c.xyy, 0.f);
+    A2[0] = __ffma2_rn(f2(-13.5f * k, 0.f), q, A2[1]);
+    A2[2] = __ffma2_rn(f2(13.5f * k, 0.f), q, A2[1]);
+  }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    const float2 mid = __ffma2_rn(f2(float(-1.0 / 3.0), float(-1.0 / 3.0)), A2[i], A0[i]);
+    const float2 te = __ffma2_rn(f2(float(2.0 / 3.0), float(2.0 / 3.0)), A2[i], A0[i]);
+    const float2 lo = sub2(te, A1[i]), hi = add2(te, A1[i]);
+    s.E[i][1] = mid.x; s.O[i][1] = mid.y;
+    s.E[i][0] = lo.x; s.O[i][0] = lo.y;
+    s.E[i][2] = hi.x; s.O[i][2] = hi.y;
+  }
+  {   // Qq = d0(cx) + cy d1 (scalar)
+    float a0[3];
+    a0[1] = (4.5f * k) * c.zz;
+    a0[0] = fmaf(-13.5f * k, c.xzz, a0[1]);
+    a0[2] = fmaf(13.5f * k, c.xzz, a0[1]);
+    const float d1 = (13.5f * k) * c.yzz;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      s.Q[i][1] = a0[i];
+      s.Q[i][0] = a0[i] - d1;
+      s.Q[i][2] = a0[i] + d1;
+    }
+  }
+}
+
 // In-plane moments {1, x, y, xx, yy, xy} of a field given on the 3x3 arrival directions, with the
 // lattice weights (1,4,1) (x) (1,4,1) (the factor 1/36 lives in the source constants).
 template <typename T> struct Red6 { T s1, sx, sy, sxx, syy, sxy; };
@@ -169,6 +231,53 @@ __device__ __forceinline__ Red6<T> reduce6(const T (&v)[3][3]) {   // v[cx+1][cy
   r.sy = fma(T(4), r1[1], r1[2] + r1[0]);
   r.syy = fma(T(4), r2[1], r2[2] + r2[0]);
   return r;
+}
+
+// Receiver side, fields E and O: gather the 8 arrivals, add the own resting direction, reduce both
+// to their six in-plane moments.  fp32: E and O travel as one float2 and the two reductions are
+// the same operation sequence on independent data, so they run as ONE sequence of packed
+// fp32x2 instructions (fma.rn.f32x2 / add.f32x2, sm_100: per component the same rounding as the
+// scalar ones, half the issue slots; K2 fp32 is issue-bound, profiles/r2_kernels_f32.txt).
+template <typename T, typename XB>
+__device__ __forceinline__ void receive_eo(const XB& xb, int tid, T ownE, T ownO, Red6<T>& rE,
+                                           Red6<T>& rO) {
+  T vE[3][3], vO[3][3];
+  vE[1][1] = ownE; vO[1][1] = ownO;
+#pragma unroll
+  for (int q = 0; q < 9; ++q) {
+    const int cx = q % 3 - 1, cy = q / 3 - 1;
+    if (cx == 0 && cy == 0) continue;
+    xb.get_eo(dir_slot(cx, cy), tid, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
+  }
+  rE = reduce6(vE);
+  rO = reduce6(vO);
+}
+template <typename XB>
+__device__ __forceinline__ void receive_eo(const XB& xb, int tid, float ownE, float ownO,
+                                           Red6<float>& rE, Red6<float>& rO) {
+  float2 v[3][3];
+  v[1][1] = make_float2(ownE, ownO);
+#pragma unroll
+  for (int q = 0; q < 9; ++q) {
+    const int cx = q % 3 - 1, cy = q / 3 - 1;
+    if (cx == 0 && cy == 0) continue;
+    v[cx + 1][cy + 1] = xb.eo[dir_slot(cx, cy)][tid];
+  }
+  float2 r0[3], r1[3], r2[3];                      // the operation order of reduce6, two lanes
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    r2[i] = add2(v[i][2], v[i][0]);
+    r1[i] = sub2(v[i][2], v[i][0]);
+    r0[i] = fma4(v[i][1], r2[i]);
+  }
+  const float2 sxx = add2(r0[2], r0[0]);
+  const float2 sx = sub2(r0[2], r0[0]);
+  const float2 s1 = fma4(r0[1], sxx);
+  const float2 sxy = sub2(r1[2], r1[0]);
+  const float2 sy = fma4(r1[1], add2(r1[2], r1[0]));
+  const float2 syy = fma4(r2[1], add2(r2[2], r2[0]));
+  rE.s1 = s1.x; rE.sx = sx.x; rE.sy = sy.x; rE.sxx = sxx.x; rE.syy = syy.x; rE.sxy = sxy.x;
+  rO.s1 = s1.y; rO.sx = sx.y; rO.sy = sy.y; rO.sxx = sxx.y; rO.syy = syy.y; rO.sxy = sxy.y;
 }
 
 // Source plane of marching index j in [-1, nz]: periodic wrap, or (walls at z = 0 / top, R19) the
@@ -295,18 +404,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
 
     if (is_out) {
       Red6<T> rE, rO, rQ;
-      {
-        T vE[3][3], vO[3][3];
-        vE[1][1] = ownE; vO[1][1] = ownO;
-#pragma unroll
-        for (int q = 0; q < 9; ++q) {
-          const int cx = q % 3 - 1, cy = q / 3 - 1;
-          if (cx == 0 && cy == 0) continue;
-          xb.get_eo(dir_slot(cx, cy), tid, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
-        }
-        rE = reduce6(vE);
-        rO = reduce6(vO);
-      }
+      receive_eo(xb, tid, ownE, ownO, rE, rO);
       if (sizeof(T) == 8) asm volatile("" ::: "memory");   // keep the Qq loads behind the E/O work
       {
         T vQ[3][3];

@@ -256,18 +256,7 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
 
     if (is_out) {
       Red6<T> rE, rO, rQ;
-      {
-        T vE[3][3], vO[3][3];
-        vE[1][1] = ownE; vO[1][1] = ownO;
-#pragma unroll
-        for (int q = 0; q < 9; ++q) {
-          const int cx = q % 3 - 1, cy = q / 3 - 1;
-          if (cx == 0 && cy == 0) continue;
-          xb.get_eo(dir_slot(cx, cy), tid, vE[cx + 1][cy + 1], vO[cx + 1][cy + 1]);
-        }
-        rE = reduce6(vE);
-        rO = reduce6(vO);
-      }
+      receive_eo(xb, tid, ownE, ownO, rE, rO);
       if (sizeof(T) == 8) asm volatile("" ::: "memory");   // keep the Qq loads behind the E/O work
       {
         T vQ[3][3];

@@ -93,19 +93,25 @@ def test_p7_p8_conservation(ref, bc):
 # ---------------------------------------------------------------- P9 -------------------
 def test_p9_laplace_law(ref):
     """Static droplet: time-averaged pressure jump = 2 sigma / R_eff (BASELINE.json north_star),
-    p = p* rho cs^2.  The p* = 0 start (R9) makes the instantaneous jump ring,
-    so a 250-step window mean is used; R_eff from the conserved droplet volume."""
+    p = p* rho cs^2.  The p* = 0 start (R9) makes the instantaneous jump ring
+    (0.2 .. 1.9 in this window), so it is averaged over steps 510..1000 (50 samples); R_eff from
+    the conserved droplet volume.  The mean does not hinge on the window: 0.992 over 510-750, 1.009
+    over 510-1000, 1.017 over 510-2000, 1.021 over 1010-2000 (measured once, 2000 steps); asserted
+    here: the whole window within 5 %, each half within 8 %."""
     cfg = I.static_droplet(32, 8.0, seed=1)
     sim, prm = make(ref, cfg["shape"], cfg["phi"], cfg["u"])
     sim.step(500)
     ratios = []
-    for _ in range(25):
+    for _ in range(50):
         sim.step(10)
-        _, p, _, phi = sim.get()
-        dp = p[phi > 0.99].mean() - p[phi < 0.01].mean()
-        r_eff = (3.0 * phi.sum() / (4.0 * np.pi)) ** (1.0 / 3.0)
+        d = sim.diag()                         # sums of p over phi > 0.99 / phi < 0.01 and counts
+        dp = d[12] / d[13] - d[14] / d[15]
+        r_eff = (3.0 * d[0] / (4.0 * np.pi)) ** (1.0 / 3.0)
         ratios.append(dp * r_eff / (2.0 * prm["sigma"]))
-    assert abs(np.mean(ratios) - 1.0) < 0.08
+    ratios = np.array(ratios)
+    assert ratios.min() < 0.7 and ratios.max() > 1.3          # it does ring: averaging is needed
+    assert abs(ratios.mean() - 1.0) < 0.05, ratios.mean()
+    assert abs(ratios[:25].mean() - 1.0) < 0.08 and abs(ratios[25:].mean() - 1.0) < 0.08
 
 
 # ---------------------------------------------------------------- P10 ------------------
