@@ -58,6 +58,10 @@ def parse():
                     help="precision of the headline value (the other one is reported beside it)")
     ap.add_argument("--flags", type=int, default=0,
                     help="validation selector (include/tslb.h TSLB_FLAG_*), 0 = production")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (weak scaling; BASELINE.json's north star, "
+                         "the default) or ONE lattice cut into z slabs with a halo exchange per "
+                         "step (strong scaling; SURVEY.md NEXT-3, paper_2501_00846_b200/slab.py)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--only", default=None, choices=[None, "f64", "f32"],
@@ -264,6 +268,48 @@ def measure(cfg, precision, args, device, ranks):
                 fma_tflops=fma)
 
 
+def measure_slab(cfg, precision, args, device, ranks):
+    """--decomp slab: this rank's z slab of the ONE global lattice; a step = tslb_step(1) on the
+    slab + the halo exchange with both neighbours (torch.distributed P2P; a local copy at N = 1).
+    Same protocol as measure(); the per-kernel split times the slab's own kernels only."""
+    import torch
+    from paper_2501_00846_b200 import binding as B, slab as S
+    nz, ny, nx = cfg["shape"]
+    sl = S.SlabSolver(nx, ny, nz, cfg["params"], ranks.rank, ranks.world, precision=precision,
+                      device=device, flags=args.flags)
+    sl.exchange = S.DistExchange(sl, ranks.rank, ranks.world, ranks.dist)
+    sl.init(cfg["phi"], cfg["u"])
+    sl.exchange()
+    d0 = sl.solver.diag()
+    sl.step(args.warmup)
+    torch.cuda.synchronize(device)
+    sampler = ClockSampler(torch.device(device).index or 0)
+    sampler.start()
+    l0 = sl.solver.launches
+    reps = []
+    for _ in range(max(1, args.repeats)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(device)
+        ranks.barrier()
+        e0.record(sl.solver.stream)
+        sl.step(args.steps)
+        e1.record(sl.solver.stream)
+        torch.cuda.synchronize(device)
+        ranks.barrier()
+        reps.append(ranks.max(e0.elapsed_time(e1)))
+    launches = (sl.solver.launches - l0) // max(1, args.repeats)
+    clocks = sampler.stop()
+    kernel_ms = sl.solver.step_timed(args.steps)
+    sl.exchange()
+    d1 = sl.solver.diag()
+    ok = all(np.isfinite(v) for v in d1.values())
+    sl.close()
+    return dict(ms=float(np.median(reps)), ms_min=float(min(reps)), reps=reps, kernel_ms=kernel_ms,
+                launches=launches, clocks=clocks, finite=ok,
+                phi_drift=abs(d1["sum_phi"] / d0["sum_phi"] - 1.0), max_u=d1["max_u"],
+                fma_tflops=B.tslb_fma_peak(precision))
+
+
 def measure_e2e(cfg, precision, args, device):
     """Host buffers through the C ABI: tslb_init_host (H2D) -> tslb_step(K) -> tslb_get_host (D2H),
     all inside the timed region."""
@@ -379,11 +425,17 @@ def main():
     periodic_fast = not (args.flags & 3) and not (bc[0] or bc[1])
     full = args.workload == "collision" and args.size == 256
     res = {}
+    slab = args.decomp == "slab"
     for prec in order:
-        r = measure(cfg, prec, args, device, ranks)
-        r["glups"] = whole_job_glups(n, args.steps, r["ms"], world)
-        r["roofline"] = roofline(r, prec, n, args.steps, peak, peak_kind, periodic_fast, full)
-        if not args.no_e2e:
+        if slab:            # one lattice over all ranks: strong scaling, per-GPU roofline
+            r = measure_slab(cfg, prec, args, device, ranks)
+            r["glups"] = whole_job_glups(n, args.steps, r["ms"], 1)
+            r["roofline"] = roofline(r, prec, n // world, args.steps, peak, peak_kind, periodic_fast, False)
+        else:
+            r = measure(cfg, prec, args, device, ranks)
+            r["glups"] = whole_job_glups(n, args.steps, r["ms"], world)
+            r["roofline"] = roofline(r, prec, n, args.steps, peak, peak_kind, periodic_fast, full)
+        if not args.no_e2e and not slab:
             r["e2e"] = measure_e2e(cfg, prec, args, device)
             r["e2e"]["value"] *= world
         res[prec] = r
@@ -406,9 +458,11 @@ def main():
                 "ms_per_step": head["ms"] / args.steps,
                 "ms_per_step_min": head["ms_min"] / args.steps,
                 "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": order[0], "data": "synthetic",
+                "scaling": "strong" if slab else "weak", "vs_baseline": None, "dtype": order[0],
+                "data": "synthetic",
                 "config": {"workload": cfg["name"], "grid": list(cfg["shape"][::-1]),
-                           "parallelism": f"replicas x{world}",
+                           "parallelism": (f"z-slabs x{world}, halo exchange per step" if slab
+                                           else f"replicas x{world}"),
                            "l2": f"state {2 * STATE_SCALARS * es0 * n / 1e9:.1f} GB ({order[0]}) >> 126 MB L2: "
                                  "inputs larger than L2, no flush needed",
                            "flags": args.flags,

@@ -105,6 +105,27 @@ int tslb_get_state(tslb_handle *h, void *pstar, void *u, void *A, void *a, void 
 int tslb_set_state(tslb_handle *h, const void *pstar, const void *u, const void *A, const void *a,
                    const void *phi);
 
+/* z-slab decomposition support (the paper's own multi-GPU runs).
+ * A slab of a lattice that is periodic along z is a handle created on nz_local + 4 planes with a
+ * periodic z axis: two ghost planes at each end.  One step needs neighbour data one plane deep
+ * for the interface update (Eq. 20) and one more for the stream-collide kernel (Eq. 8), so ONE
+ * exchange of two planes per face and step keeps planes [2, nz-2) exact; what the step writes into
+ * the ghost planes is overwritten by the next exchange.
+ *   tslb_halo_pack(h, face, buf):   copy the owned planes next to the face, [2, 4) for face 0
+ *                                   (low z) or [nz-4, nz-2) for face 1, of every internal array
+ *                                   (13 moments, phi, the flux of Eq. 20: 17 scalars per node)
+ *                                   into the DEVICE buffer buf of tslb_halo_bytes(h) bytes;
+ *   tslb_halo_unpack(h, face, buf): write such a buffer into the ghost planes [0, 2) (face 0)
+ *                                   or [nz-2, nz) (face 1).
+ * The low neighbour's face-1 buffer goes into this slab's face 0 and vice versa.  The format of
+ * the buffer is private to the library (same size, precision and flags on both sides).  One
+ * launch each on the handle's stream, no synchronisation; after tslb_init and after every
+ * tslb_step(1).  Needs a periodic z axis of >= 6 planes and the lean kernel pair (periodic x, y;
+ * flags NAIVE / GENERIC unset).  paper_2501_00846_b200/slab.py drives it over torch.distributed. */
+size_t tslb_halo_bytes(const tslb_handle *h);
+int tslb_halo_pack(tslb_handle *h, int face, void *buf);
+int tslb_halo_unpack(tslb_handle *h, int face, const void *buf);
+
 /* On-device diagnostics: box reductions of the current state, the
  * quantities behind the paper's validation plots (centre-of-mass velocity of a rising bubble,
  * Fig. 4) and BASELINE.json's checks (sum(phi) conserved; Laplace's law

@@ -22,6 +22,7 @@ DIAG_NAMES = ("sum_phi", "sum_pstar", "max_u", "sum_phi_x", "sum_phi_y", "sum_ph
 SYMBOLS = ("tslb_workspace_bytes", "tslb_create", "tslb_init", "tslb_step", "tslb_get",
            "tslb_get_state", "tslb_set_state", "tslb_init_host", "tslb_get_host", "tslb_step_timed",
            "tslb_launch_count", "tslb_diag", "tslb_diag_host", "tslb_diag_static", "tslb_fma_peak",
+           "tslb_halo_bytes", "tslb_halo_pack", "tslb_halo_unpack",
            "tslb_destroy", "tslb_last_error")
 
 
@@ -73,6 +74,10 @@ def load():
     lib.tslb_diag_host.argtypes = [vp, C.POINTER(C.c_double)]
     lib.tslb_diag_static.argtypes = [vp, vp]
     lib.tslb_fma_peak.argtypes = [C.c_int, vp, C.POINTER(C.c_double)]
+    lib.tslb_halo_bytes.argtypes = [vp]
+    lib.tslb_halo_bytes.restype = C.c_size_t
+    lib.tslb_halo_pack.argtypes = [vp, C.c_int, vp]
+    lib.tslb_halo_unpack.argtypes = [vp, C.c_int, vp]
     lib.tslb_launch_count.argtypes = [vp]
     lib.tslb_launch_count.restype = C.c_longlong
     lib.tslb_destroy.argtypes = [vp]
@@ -198,6 +203,18 @@ class Solver:
         self._call("tslb_set_state", t["pstar"].data_ptr(), t["u"].data_ptr(), t["A"].data_ptr(),
                    t["a"].data_ptr(), t["phi"].data_ptr())
         self.stream.synchronize()          # the arrays may be temporaries
+
+    def halo_buffer(self):
+        """A device tensor of tslb_halo_bytes for tslb_halo_pack / tslb_halo_unpack."""
+        n = int(self.lib.tslb_halo_bytes(self._h))
+        es = 8 if self.dtype == self.torch.float64 else 4
+        return self.torch.empty(n // es, dtype=self.dtype, device=self.device)
+
+    def halo_pack(self, face, buf):
+        self._call("tslb_halo_pack", int(face), buf.data_ptr())
+
+    def halo_unpack(self, face, buf):
+        self._call("tslb_halo_unpack", int(face), buf.data_ptr())
 
     def diag(self):
         """tslb_diag_host: dict of the TSLB_D_* box reductions (synchronises the stream)."""

@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -214,6 +215,42 @@ __global__ void __launch_bounds__(256) k_fma_peak(T seed) {
   if (s == T(-12345.678)) g_fma_sink[sizeof(T) == 8] = double(s);    // never true: keeps the chains
 }
 
+// ---- z-slab halo exchange support (NEXT-3) --------------------------------------------------
+// first plane of the face's source (pack) or destination (unpack) range
+int halo_first_plane(const tslb_handle* h, int face, bool pack) {
+  const int d = tslb::HALO_DEPTH;
+  if (pack) return face == 0 ? d : h->nz - 2 * d;
+  return face == 0 ? 0 : h->nz - d;
+}
+template <typename T>
+tslb::HaloSegs halo_segments(const tslb_handle* h, int z) {
+  constexpr int W = tslb::VecOf<T>::W, KV = 12 / W;
+  const long long pl = (long long)h->nx * h->ny, N = h->stride, d = tslb::HALO_DEPTH;
+  tslb::HaloSegs sg;
+  sg.n = 0;
+  auto add = [&](long long off, long long len, int in_q) {
+    sg.arr_off[sg.n] = off; sg.len[sg.n] = len; sg.in_q[sg.n] = in_q; ++sg.n;
+  };
+  for (int k = 0; k < KV; ++k) add((long long)k * W * N + (long long)z * pl * W, d * pl * W, 0);
+  add(12 * N + (long long)z * pl, d * pl, 0);            // az
+  add(13 * N + (long long)z * pl, d * pl, 0);            // phi
+  for (int k = 0; k < 3; ++k) add((long long)k * N + (long long)z * pl, d * pl, 1);   // flux Q
+  return sg;
+}
+template <typename T, bool PACK>
+int halo_launch(tslb_handle* h, int face, void* buf) {
+  const tslb::HaloSegs sg = halo_segments<T>(h, halo_first_plane(h, face, PACK));
+  long long total = 0;
+  for (int i = 0; i < sg.n; ++i) total += sg.len[i];
+  const unsigned blocks = unsigned(std::min<long long>((total + 255) / 256, 148LL * 16));
+  tslb::k_halo_copy<T, PACK><<<blocks, 256, 0, h->stream>>>(
+      sg, reinterpret_cast<T*>(h->buf[h->cur]), reinterpret_cast<T*>(h->scratch),
+      static_cast<T*>(buf));
+  h->launches += 1;
+  CUDA_TRY(cudaGetLastError());
+  return TSLB_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -304,6 +341,35 @@ int tslb_set_state(tslb_handle* h, const void* pstar, const void* u, const void*
   CUDA_TRY(cudaGetLastError());
   h->inited = true;
   return TSLB_OK;
+}
+
+size_t tslb_halo_bytes(const tslb_handle* h) {
+  if (!h) return 0;
+  return size_t(17) * tslb::HALO_DEPTH * size_t(h->nx) * h->ny * h->es;
+}
+
+static int halo_check(const tslb_handle* h, int face, const void* buf, const char* who) {
+  if (!h || !buf || (face != 0 && face != 1)) return fail(TSLB_EINVAL, "%s: bad argument", who);
+  if (!h->inited) return fail(TSLB_ESTATE, "%s before tslb_init", who);
+  if (h->prm.bc[2] != TSLB_BC_PERIODIC || h->nz < 3 * tslb::HALO_DEPTH)
+    return fail(TSLB_EINVAL, "%s: needs a periodic z axis of at least 6 planes", who);
+  if (h->prm.flags & (TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC))
+    return fail(TSLB_EINVAL, "%s: the flux planes belong to the lean pair (flags NAIVE / GENERIC unset)", who);
+  return TSLB_OK;
+}
+
+int tslb_halo_pack(tslb_handle* h, int face, void* buf) {
+  int rc = halo_check(h, face, buf, "tslb_halo_pack");
+  if (rc != TSLB_OK) return rc;
+  return h->prm.precision == TSLB_F64 ? halo_launch<double, true>(h, face, buf)
+                                      : halo_launch<float, true>(h, face, buf);
+}
+
+int tslb_halo_unpack(tslb_handle* h, int face, const void* buf) {
+  int rc = halo_check(h, face, buf, "tslb_halo_unpack");
+  if (rc != TSLB_OK) return rc;
+  return h->prm.precision == TSLB_F64 ? halo_launch<double, false>(h, face, const_cast<void*>(buf))
+                                      : halo_launch<float, false>(h, face, const_cast<void*>(buf));
 }
 
 // partial sums into `rows` (device scratch of diag_rows(nodes) rows), result into `out` (device)

@@ -268,3 +268,34 @@ __global__ void __launch_bounds__(256) k_get_state(DevParams<T> P, long long nod
   if (phi) phi[idx] = S[F_PHI * P.N + idx];
 }
 }  // namespace tslb
+
+namespace tslb {
+// ---- halo planes of the z-slab decomposition -----------
+// A slab keeps HALO_DEPTH ghost planes at each end of its z range.  Every internal array (the
+// 128-bit field-vector planes, az, phi of the current state buffer, the three flux planes) is
+// contiguous over consecutive z planes, so the planes of one face are a handful of contiguous
+// segments: one kernel copies them to / from a packed buffer, element by element.
+constexpr int HALO_DEPTH = 2;      // K1 reaches one plane, K2 one more: one exchange per step
+constexpr int HALO_MAXSEG = 12;
+struct HaloSegs {
+  int n;
+  long long arr_off[HALO_MAXSEG];   // element offset of the segment inside the state buffer (or
+                                    // inside the flux scratch when in_q is set)
+  long long len[HALO_MAXSEG];       // elements
+  int in_q[HALO_MAXSEG];
+};
+template <typename T, bool PACK>
+__global__ void __launch_bounds__(256) k_halo_copy(HaloSegs sg, T* __restrict__ state,
+                                                   T* __restrict__ q, T* __restrict__ buf) {
+  long long total = 0;
+  for (int i = 0; i < sg.n; ++i) total += sg.len[i];
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < total;
+       e += (long long)gridDim.x * blockDim.x) {
+    long long r = e;
+    int i = 0;
+    while (r >= sg.len[i]) { r -= sg.len[i]; ++i; }
+    T* a = (sg.in_q[i] ? q : state) + sg.arr_off[i] + r;
+    if (PACK) buf[e] = *a; else *a = buf[e];
+  }
+}
+}  // namespace tslb
