@@ -187,11 +187,14 @@ cudaError_t launch_k1_flux(const DevParams<T>& P, const T* S, const T* Q, T* D, 
 }
 
 // Planes per block such that the grid fills whole waves of `slots` resident blocks: among the
-// chunk counts that give between 16 and 64 planes per block, the one with the best last wave.
+// chunk counts that give between 4 and 64 planes per block, the one with the best product of
+// last-wave efficiency and priming efficiency (2 extra source planes per chunk).  Small lattices
+// (fewer blocks than slots) thereby get short chunks: their step time is the latency of one
+// block's march, not throughput.
 inline int balanced_zchunk(long long tiles_xy, int nz, int slots) {
   int best = 32;
   double best_eff = -1.0;
-  for (int nch = (nz + 63) / 64; nch <= (nz + 15) / 16; ++nch) {
+  for (int nch = (nz + 63) / 64; nch <= (nz + 3) / 4; ++nch) {
     const int zc = (nz + nch - 1) / nch;
     const long long blocks = tiles_xy * ((nz + zc - 1) / zc);
     const double waves = double(blocks) / slots;
@@ -262,7 +265,7 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
     constexpr int minb = sizeof(T) == 8 ? 1 : 2;
     const long long tiles = (long long)((P.nx + 31) / 32) * ((P.ny + 7) / 8);
     const bool deep = tiles * ((P.nz + 63) / 64) >= 3LL * 148 * minb;
-    const int zc = deep ? 64 : 32;
+    const int zc = deep ? 64 : balanced_zchunk(tiles, P.nz, 148 * minb);
     // TMA tensor staging two planes ahead: fp64 production on deep grids with full tile rows
     // (0.79 ms on 256^3 against 0.85 ms with cp.async); elsewhere only when asked for
     bool want_tma = tc && tma_usable(P) && !(flags & SEL_K2_CPASYNC) &&

@@ -28,7 +28,7 @@ CASES = {
     # ---- configs[3]: head-on collision at the graded 256^3
     "collision256": (lambda: I.head_on_collision(n=256), [1, 10, 50, 100, 200, 500, 1000]),
     # ---- configs[4]: emulsion at 384^3 (the oracle needs ~40 GB there; 512^3 does not fit)
-    "emulsion384": (lambda: I.emulsion_sweep(n=384), [1, 5, 10]),
+    "emulsion384": (lambda: I.emulsion_sweep(n=384), [1, 5, 10, 20, 50]),
     # ---- NEXT-2: off-axis collision, impact parameter 0.4, at 128^3
     "offaxis128": (lambda: I.off_axis_collision(n=128, impact=0.4), [1, 10, 100, 300]),
 }
