@@ -58,6 +58,8 @@ def parse():
                     help="precision of the headline value (the other one is reported beside it)")
     ap.add_argument("--flags", type=int, default=0,
                     help="validation selector (include/tslb.h TSLB_FLAG_*), 0 = production")
+    ap.add_argument("--bc", default=None,
+                    help="override the boundary types, e.g. 1,1,1 = walls on x, y and z")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (weak scaling; BASELINE.json's north star, "
                          "the default) or ONE lattice cut into z slabs with a halo exchange per "
@@ -418,6 +420,9 @@ def main():
 
     cfg = make_workload(args.size, args.workload)
     cfg["_size"], cfg["_kind"] = args.size, args.workload
+    if args.bc:
+        cfg["params"] = dict(cfg["params"], bc=tuple(int(v) for v in args.bc.split(",")))
+        cfg["name"] += "_bc" + args.bc.replace(",", "")
     n = int(np.prod(cfg["shape"]))
     peak, peak_kind = peaks()
     order = [args.only] if args.only else [args.precision, "f32" if args.precision == "f64" else "f64"]

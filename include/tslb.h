@@ -120,8 +120,8 @@ int tslb_set_state(tslb_handle *h, const void *pstar, const void *u, const void 
  * The low neighbour's face-1 buffer goes into this slab's face 0 and vice versa.  The format of
  * the buffer is private to the library (same size, precision and flags on both sides).  One
  * launch each on the handle's stream, no synchronisation; after tslb_init and after every
- * tslb_step(1).  Needs a periodic z axis of >= 6 planes and the lean kernel pair (periodic x, y;
- * flags NAIVE / GENERIC unset).  paper_2501_00846_b200/slab.py drives it over torch.distributed. */
+ * tslb_step(1).  Needs a periodic z axis of >= 6 planes, periodic x and y, and flags NAIVE /
+ * GENERIC unset (the flux planes belong to the lean kernel pair).  paper_2501_00846_b200/slab.py drives it over torch.distributed. */
 size_t tslb_halo_bytes(const tslb_handle *h);
 int tslb_halo_pack(tslb_handle *h, int face, void *buf);
 int tslb_halo_unpack(tslb_handle *h, int face, const void *buf);

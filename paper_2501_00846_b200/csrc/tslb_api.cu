@@ -353,6 +353,9 @@ static int halo_check(const tslb_handle* h, int face, const void* buf, const cha
   if (!h->inited) return fail(TSLB_ESTATE, "%s before tslb_init", who);
   if (h->prm.bc[2] != TSLB_BC_PERIODIC || h->nz < 3 * tslb::HALO_DEPTH)
     return fail(TSLB_EINVAL, "%s: needs a periodic z axis of at least 6 planes", who);
+  if (h->prm.bc[0] != TSLB_BC_PERIODIC || h->prm.bc[1] != TSLB_BC_PERIODIC)
+    return fail(TSLB_EINVAL, "%s: walls on x or y need a deeper halo than two planes (the "
+                "interface kernel recomputes the normals there)", who);
   if (h->prm.flags & (TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC))
     return fail(TSLB_EINVAL, "%s: the flux planes belong to the lean pair (flags NAIVE / GENERIC unset)", who);
   return TSLB_OK;

@@ -300,7 +300,8 @@ __device__ __forceinline__ int source_plane(int j, int nz, int bcz) {
 // its cz = -1 combination on plane nz-1, and the rest falls on planes that do not exist.
 template <typename T, int TX, int TY, typename XB>
 __device__ __forceinline__ void publish(XB& xb, const SrcFields<T>& sf, bool ghost, bool is_main,
-                                        unsigned need, int rb, T& ownE, T& ownO, T& ownQ) {
+                                        unsigned need, int rb, T& ownE, T& ownO, T& ownQ,
+                                        unsigned wmask = 0u) {
   if (!ghost) {
     ownE = sf.E[1][1]; ownO = sf.O[1][1]; ownQ = sf.Q[1][1];
 #pragma unroll
@@ -316,15 +317,55 @@ __device__ __forceinline__ void publish(XB& xb, const SrcFields<T>& sf, bool gho
     for (int q = 0; q < 9; ++q) {
       const int cx = q % 3 - 1, cy = q / 3 - 1;
       if (cx == 0 && cy == 0) continue;
+      if (wmask >> dir_slot(cx, cy) & 1u) continue;      // owned by the in-plane wall accounting
       xb.put(dir_slot(cx, cy), rb, sf.E[1 - cx][1 - cy], -sf.O[1 - cx][1 - cy], sf.Q[1 - cx][1 - cy]);
     }
   }
 }
 
+// Walls on the TILE axes x, y (halfway bounce-back, R19).  A receiver r next to such a wall has
+// in-plane arrival directions a whose source r - a lies beyond the wall (bit dir_slot(a) of
+// wmask).  For those, all three vertical directions bounce: the arrival (a, cz) at plane k is the
+// node's own fpost(-a, -cz) of plane k, i.e. the fields (E(-a), -O(-a), Qq(-a)) of the node's OWN
+// plane-k source evaluation -- not distributed over planes k-1, k, k+1 like a neighbour's, but
+// all three landing on plane k.  Summed over cz with the lattice weights (1, 4, 1):
+//   in-plane moments {1,x,y,xx,yy,xy}: 6 red(E')        (the Qq parts cancel: 2/3 - 4/3 + 2/3 = 0)
+//   mz, xz, yz: 2 red(O').{1,x,y}        zz: 2 red(E' + 2/3 Qq').1
+// which is added to the accumulators of plane k when the node's own fields of plane k exist
+// (iteration j = k, before the barrier).  The receiver slots of those directions are zeroed once
+// and never written by anybody, so the regular reduction adds nothing for them.
+template <typename T>
+__device__ __forceinline__ void wall_bounce(const SrcFields<T>& sf, unsigned wmask, T (&aB)[6],
+                                            T (&zB)[3], T& zcB) {
+  T bE[3][3], bO[3][3], bQ[3][3];
+#pragma unroll
+  for (int q = 0; q < 9; ++q) {
+    const int cx = q % 3 - 1, cy = q / 3 - 1;
+    const bool on = (cx != 0 || cy != 0) && (wmask >> dir_slot(cx, cy) & 1u);
+    bE[cx + 1][cy + 1] = on ? sf.E[1 - cx][1 - cy] : T(0);
+    bO[cx + 1][cy + 1] = on ? -sf.O[1 - cx][1 - cy] : T(0);
+    bQ[cx + 1][cy + 1] = on ? sf.Q[1 - cx][1 - cy] : T(0);
+  }
+  const Red6<T> e = reduce6(bE), o = reduce6(bO), qq = reduce6(bQ);
+  aB[0] = fma(T(6), e.s1, aB[0]);   aB[1] = fma(T(6), e.sx, aB[1]);   aB[2] = fma(T(6), e.sy, aB[2]);
+  aB[3] = fma(T(6), e.sxx, aB[3]);  aB[4] = fma(T(6), e.syy, aB[4]);  aB[5] = fma(T(6), e.sxy, aB[5]);
+  zB[0] = fma(T(2), o.s1, zB[0]);   zB[1] = fma(T(2), o.sx, zB[1]);   zB[2] = fma(T(2), o.sy, zB[2]);
+  zcB += T(2) * (fma(T(2.0 / 3.0), qq.s1, e.s1) - o.s1);
+}
+
+// mirrored (wall) or wrapped (periodic) index of a ring coordinate g in [-1, n]
+__device__ __forceinline__ int ring_source(int g, int n, int bc) {
+  if (g < 0) return bc ? -1 - g : g + n;
+  if (g >= n) return bc ? 2 * n - 1 - g : g - n;
+  return g;
+}
+
 // cp.async staging NSTAGE >= 1 planes ahead: each thread copies the 14 scalars of ITS OWN node
 // for plane j + NSTAGE straight into a private shared-memory slot (StageBuf, tslb_device.cuh)
 // and picks them up NSTAGE iterations later; only cp.async.wait_group is needed.
-template <typename T, int TX, int TY, int MINB, int NSTAGE>
+// WXY: walls on x or y are possible (wall_bounce); false compiles the accounting out so that the
+// all-periodic instantiations keep their registers
+template <typename T, int TX, int TY, int MINB, int NSTAGE, bool WXY = false>
 __global__ void __launch_bounds__((TileMap<TX, TY, 1>::NTHREADS), MINB)
 k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D,
                       T* __restrict__ Qout, int zchunk) {
@@ -345,14 +386,33 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   const int z1 = min(P.nz, z0 + zchunk);
   const int c = M::cell(lx, ly);
   const int rb = ly * TX + lx;                                  // index as a receiver (main: tid)
-  const unsigned need = mapped ? dir_mask<TX, TY>(lx, ly) : 0u; // directions somebody reads
   const bool in_ring = mapped && gx >= -1 && gx <= P.nx && gy >= -1 && gy <= P.ny;
   const bool is_out = tid < M::NMAIN && gx < P.nx && gy < P.ny;
-  const int sx = gx < 0 ? gx + P.nx : (gx >= P.nx ? gx - P.nx : gx);      // periodic wrap
-  const int sy = gy < 0 ? gy + P.ny : (gy >= P.ny ? gy - P.ny : gy);
+  // a ring cell beyond a wall of the tile axes is no source: it only supplies the mirrored
+  // phi^{n+1} ghost (R19); every other ring cell is the periodic image
+  const bool beyond = WXY && ((P.bcx && (gx < 0 || gx >= P.nx)) || (P.bcy && (gy < 0 || gy >= P.ny)));
+  const unsigned need = (mapped && !beyond) ? dir_mask<TX, TY>(lx, ly) : 0u;   // directions somebody reads
+  const int sx = ring_source(gx, P.nx, WXY ? P.bcx : 0);
+  const int sy = ring_source(gy, P.ny, WXY ? P.bcy : 0);
   const int plane = P.nx * P.ny;
   const int col = in_ring ? sx + P.nx * sy : 0;
   const T* phin = D + F_PHI * P.N;
+  // receiver's in-plane arrival directions whose source lies beyond a wall (wall_bounce)
+  unsigned wmask = 0u;
+  if (WXY && is_out && (P.bcx || P.bcy)) {
+#pragma unroll
+    for (int q = 0; q < 9; ++q) {
+      const int cx = q % 3 - 1, cy = q / 3 - 1;
+      if (cx == 0 && cy == 0) continue;
+      const bool out = (P.bcx && ((cx == 1 && gx == 0) || (cx == -1 && gx == P.nx - 1))) ||
+                       (P.bcy && ((cy == 1 && gy == 0) || (cy == -1 && gy == P.ny - 1)));
+      if (out) {
+        wmask |= 1u << dir_slot(cx, cy);
+        sm.buf[0].put(dir_slot(cx, cy), tid, T(0), T(0), T(0));     // nobody else writes these
+        sm.buf[1].put(dir_slot(cx, cy), tid, T(0), T(0), T(0));
+      }
+    }
+  }
 
   // cp.async pipeline: one commit group per plane, issued by every thread (possibly empty)
   auto stage_issue = [&](int j, int slot) {
@@ -382,10 +442,11 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   // j-1, completed in iteration j; "B" = destination plane j), so the marching loop is unrolled
   // by two and no register is moved to shift the pipeline.
   T acc0[6] = {}, acc1[6] = {}, zo0[3] = {}, zo1[3] = {}, u0[3] = {}, u1[3] = {};
+  T zc0 = 0, zc1 = 0;                          // zz of the in-plane wall bounce (wall_bounce)
   T ph_m = 0, ph_0 = 0, ph_p = 0;
 
   auto body = [&](const int j, const int slot, XB& xb, T (&aA)[6], T (&aB)[6],
-                  T (&zA)[3], T (&zB)[3], const T (&uPrev)[3], T (&uCur)[3]) {
+                  T (&zA)[3], T (&zB)[3], T& zcA, T& zcB, const T (&uPrev)[3], T (&uCur)[3]) {
     T ownE = 0, ownO = 0, ownQ = 0;
     ph_m = ph_0; ph_0 = ph_p;
     if (in_ring) {
@@ -396,7 +457,9 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
       SrcFields<T> sf;
       const Coef<T> cf = coef_from13(cur);
       source_fields(cf, sf);
-      publish<T, TX, TY>(xb, sf, P.bcz && (j < 0 || j >= P.nz), tid < M::NMAIN, need, rb, ownE, ownO, ownQ);
+      const bool ghost = P.bcz && (j < 0 || j >= P.nz);
+      publish<T, TX, TY>(xb, sf, ghost, tid < M::NMAIN, need, rb, ownE, ownO, ownQ, wmask);
+      if (WXY && wmask != 0u && !ghost) wall_bounce(sf, wmask, aB, zB, zcB);
       xb.put_pd(c, fma(T(4), ph_0, ph_m + ph_p), ph_p - ph_m);
     }
     stage_issue(j + NSTAGE, slot);             // refill the slot just consumed
@@ -437,6 +500,7 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
         m.xx = aA[3]; m.yy = aA[4]; m.xy = aA[5];
         m.mz = zA[0] - dn[0]; m.xz = zA[1] - dn[1]; m.yz = zA[2] - dn[2];
         m.zz = zA[0] + dn[0];
+        if (WXY) m.zz += zcA;
         if (sizeof(T) == 8) asm volatile("" ::: "memory");
         // separable gradient / Laplacian of phi^{n+1} at plane k (Eq. 18, repaired Eq. 19)
         T rs[3], rd[3], zs[3];
@@ -470,16 +534,17 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
       for (int i = 0; i < 6; ++i) aA[i] = up[i];
 #pragma unroll
       for (int i = 0; i < 3; ++i) zA[i] = up[i];
+      zcA = T(0);
     }
   };
 
   int slot = 0;                                 // staging slot of plane j: (j - z0 + 1) % NSTAGE
   auto next_slot = [&]() { if (NSTAGE > 1) slot = (slot + 1 == NSTAGE) ? 0 : slot + 1; };
   for (int j = z0 - 1; j <= z1; j += 2) {
-    body(j, slot, sm.buf[0], acc0, acc1, zo0, zo1, u0, u1);
+    body(j, slot, sm.buf[0], acc0, acc1, zo0, zo1, zc0, zc1, u0, u1);
     next_slot();
     if (j + 1 <= z1) {
-      body(j + 1, slot, sm.buf[1], acc1, acc0, zo1, zo0, u1, u0);
+      body(j + 1, slot, sm.buf[1], acc1, acc0, zo1, zo0, zc1, zc0, u1, u0);
       next_slot();
     }
   }

@@ -36,11 +36,11 @@ inline cudaError_t prepare(K kernel, size_t smem, bool (&ready)[kMaxDev]) {
 }
 
 // ---- lean periodic stream-collide kernel, cp.async staging NSTAGE planes ahead ---------------
-template <typename T, int TY, int MINB, int NSTAGE, int TX = 32>
+template <typename T, int TY, int MINB, int NSTAGE, bool WXY = false, int TX = 32>
 cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
                         int zc = ZCHUNK) {
   using M = TileMap<TX, TY, 1>;
-  auto kernel = k_stream_collide_fast<T, TX, TY, MINB, NSTAGE>;
+  auto kernel = k_stream_collide_fast<T, TX, TY, MINB, NSTAGE, WXY>;
   const size_t smem = sizeof(K2FastSmem<T, M::CELLS, M::NMAIN>) + NSTAGE * sizeof(StageBuf<T, M::CELLS>);
   static bool ready[kMaxDev] = {};
   cudaError_t e = prepare(kernel, smem, ready);
@@ -233,18 +233,17 @@ enum { SEL_GENERIC = 2, SEL_K2_CPASYNC = 4, SEL_K2_TMA = 8, SEL_K1_FLUX = 16 };
 template <typename T>
 int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
                       long long* launches, const Marker& mk, int flags, TmaCache* tc = nullptr) {
-  const bool walls = P.bcx || P.bcy || P.bcz;
-  // The lean pair serves periodic tile axes (x, y); walls on the MARCHING axis z (configs[2]:
-  // no-slip floor and lid) cost it two ghost planes per column (bounce-back in publish(), ghost
-  // flux in the row kernel).  Walls on x or y, or rows that the row kernel cannot vectorise on a
-  // box with walls, run the wall-capable pair.
+  const bool side_walls = P.bcx || P.bcy;
+  const bool forced = (flags & SEL_GENERIC) != 0;
   const bool row_ok = P.nx % RowVec<T>::V == 0;
-  const bool generic = P.bcx || P.bcy || (P.bcz && !row_ok) || (flags & SEL_GENERIC);
   cudaError_t e;
-  // ---- K1
-  if (generic) {
-    // wall-capable: normals recomputed on a ring of depth 2 (the two parts of the flux mirror
-    // differently at a wall, so the flux form cannot serve walls)
+  // ---- K1 (interface tracking).  The flux-form kernels serve periodic tile axes; the row kernel
+  // also walls on the marching axis z (ghost flux planes).  Walls on x or y, where the two parts
+  // of the flux mirror differently, run the wall-capable kernel (normals recomputed on a ring of
+  // depth 2), which hands no flux over: K2 then writes none.
+  const bool k1_tiled = forced || side_walls || (P.bcz && !row_ok);
+  if (k1_tiled) {
+    const bool walls = side_walls || P.bcz;
     e = walls ? launch_k1w<T, true>(P, S, D, stream) : launch_k1w<T, false>(P, S, D, stream);
   } else if (row_ok && (P.bcz || !(flags & SEL_K1_FLUX))) {
     e = launch_k1_row<T>(P, S, Q, D, stream);
@@ -253,8 +252,12 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
   }
   if (e != cudaSuccess) return int(e);
   mk.mark(1);
-  // ---- K2
-  if (generic) {
+  // ---- K2 (stream-collide-moments-forces): the lean kernel unless the wall-capable one is
+  // forced; walls on z cost it two ghost planes per column (publish()), walls on x or y the
+  // bounce accounting of the wall-adjacent receivers (wall_bounce, cp.async staging only)
+  T* Qk2 = k1_tiled ? nullptr : Q;
+  if (forced) {
+    const bool walls = side_walls || P.bcz;
     // cp.async staging pays in fp32 (0.75 vs 1.16 ms on 256^3) but not in fp64 (1.91 vs 1.83 ms)
     constexpr int NS = sizeof(T) == 8 ? 0 : 1;
     e = walls ? launch_generic<T, true, NS>(P, S, D, stream)
@@ -268,14 +271,20 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
     const int zc = deep ? 64 : balanced_zchunk(tiles, P.nz, 148 * minb);
     // TMA tensor staging two planes ahead: fp64 production on deep grids with full tile rows
     // (0.79 ms on 256^3 against 0.85 ms with cp.async); elsewhere only when asked for
-    bool want_tma = tc && tma_usable(P) && !(flags & SEL_K2_CPASYNC) &&
+    bool want_tma = tc && tma_usable(P) && !side_walls && !(flags & SEL_K2_CPASYNC) &&
                     ((flags & SEL_K2_TMA) || (sizeof(T) == 8 && deep));
     e = cudaErrorNotSupported;
-    if (want_tma) e = launch_tma<T, 8, minb, 2>(P, S, D, Q, stream, zc, tc);
+    if (want_tma) e = launch_tma<T, 8, minb, 2>(P, S, D, Qk2, stream, zc, tc);
     if (e == cudaErrorNotSupported) {          // not wanted, or no tensor-map encoder: cp.async
-      if constexpr (sizeof(T) == 8) e = launch_fast<T, 8, 1, 1>(P, S, D, Q, stream, zc);
-      else e = deep ? launch_fast<T, 8, 2, 2>(P, S, D, Q, stream, zc)
-                    : launch_fast<T, 8, 2, 1>(P, S, D, Q, stream, zc);
+      if (side_walls) {
+        if constexpr (sizeof(T) == 8) e = launch_fast<T, 8, 1, 1, true>(P, S, D, Qk2, stream, zc);
+        else e = launch_fast<T, 8, 2, 1, true>(P, S, D, Qk2, stream, zc);
+      } else if constexpr (sizeof(T) == 8) {
+        e = launch_fast<T, 8, 1, 1>(P, S, D, Qk2, stream, zc);
+      } else {
+        e = deep ? launch_fast<T, 8, 2, 2>(P, S, D, Qk2, stream, zc)
+                 : launch_fast<T, 8, 2, 1>(P, S, D, Qk2, stream, zc);
+      }
     }
   }
   mk.mark(2);

@@ -219,6 +219,23 @@ def test_resume_from_a_state_dump(precision, tol):
         b.close()
 
 
+@pytest.mark.parametrize("bc", [(1, 0, 0), (0, 1, 0), (1, 1, 0), (1, 1, 1), (0, 1, 1)])
+@pytest.mark.parametrize("sel", ["auto", "generic"])
+def test_side_walls_on_the_lean_kernel(ref, bc, sel):
+    """Walls on the tile axes x / y: the lean stream-collide kernel with the bounce accounting of
+    the wall-adjacent receivers (wall_bounce) + the wall-capable interface kernel; the
+    wall-capable pair is the cross-check.  Three x tiles, five y tiles, two z chunks, ragged;
+    droplets sitting in a corner, on an edge and on a face, gravity oblique to every wall."""
+    shape = (40, 37, 70)                                         # (nz, ny, nx)
+    prm = I.base_params(bc=bc, body_accel=(1e-5, -2e-5, 1.5e-5))
+    phi = I.sphere_profile(shape, (2.3, 1.8, 3.1), 7.0, 4.0, bc)            # low corner
+    phi += I.sphere_profile(shape, (67.2, 18.4, 37.6), 6.0, 4.0, bc)        # high x face / top
+    phi += I.sphere_profile(shape, (35.5, 35.1, 20.3), 5.0, 4.0, bc)        # high y face
+    cfg = dict(name="side_walls", shape=shape, params=prm, phi=np.minimum(phi, 1.0),
+               u=I.noise_u(shape, 1e-3, 59))
+    _check_both_precisions(ref, cfg, [1, 2, 12], SELECTORS[sel], f"side walls {bc}/{sel}")
+
+
 def test_stray_flag_bits_are_rejected():
     from paper_2501_00846_b200 import binding as B
     cfg = I.static_droplet(16, 4.0, seed=2)
