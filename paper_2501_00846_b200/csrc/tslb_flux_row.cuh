@@ -1,4 +1,4 @@
-// tslb_flux_row.cuh -- interface tracking (Eq. 20) in flux form, ROW kernel (all-periodic boxes).
+// tslb_flux_row.cuh -- interface tracking (Eq. 20) in flux form, ROW kernel (periodic axes and walls).
 //
 // Same arithmetic as tslb_flux.cuh (phi^{n+1} = phi - div Q + D lap(phi), Eq. 18 / repaired
 // Eq. 19, R10, R16), other work distribution.  The kernel moves only 5 scalars per update, so it
@@ -62,7 +62,9 @@ __device__ __forceinline__ T zsum141(T v, T& a, T& b) {
   return r;
 }
 
-template <typename T, int TY, int MINB, int NSTAGE>
+// WXY: walls on x or y are possible; false compiles their ghost handling out (the periodic and
+// z-wall instantiations keep their registers)
+template <typename T, int TY, int MINB, int NSTAGE, bool WXY = false>
 __global__ void __launch_bounds__((TY + 3) * 32, MINB)
 k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ Q,
                  T* __restrict__ phin, int zchunk) {
@@ -89,40 +91,51 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
   const int side = lane & 1;
   const int gy = blockIdx.y * TY + row - 1;
   const bool row_used = row < ROWS && gy <= P.ny;  // rows beyond the +1 halo of a ragged tile idle
-  const int sy = gy < 0 ? gy + P.ny : (gy >= P.ny ? gy - P.ny : gy);
+  // source of a position beyond the lattice: the periodic image, or (wall, R19) the mirrored node
+  auto src = [](int g, int n, int bc, int& crossed) {
+    crossed = 0;
+    if (g < 0) { crossed = bc; return bc ? -1 - g : g + n; }
+    if (g >= n) { crossed = bc; return bc ? 2 * n - 1 - g : g - n; }
+    return g;
+  };
+  int kx_ = 0, ky_ = 0;                            // this thread's nodes lie beyond an x / y wall
+  const int sy = src(gy, P.ny, WXY ? P.bcy : 0, ky_);
   int sx;                                          // first (row warps) or only (extra warp) column
-  if (xhalo) {
-    sx = side == 0 ? gx0 - 1 : gx0 + nact * V;
-    sx = sx < 0 ? sx + P.nx : (sx >= P.nx ? sx - P.nx : sx);
-  } else {
-    sx = gx0 + lane * V;
-  }
+  if (xhalo) sx = src(side == 0 ? gx0 - 1 : gx0 + nact * V, P.nx, WXY ? P.bcx : 0, kx_);
+  else sx = gx0 + lane * V;
+  const int kx = WXY ? kx_ : 0, ky = WXY ? ky_ : 0;
   const bool active = row_used && (xhalo || lane < nact);
   const bool is_out = !xhalo && active && row >= 1 && row <= TY && gy < P.ny;
   const int col = active ? sx + P.nx * sy : 0;
 
-  // Walls on the marching axis (R19): the ghost plane j = -1 / nz is the mirrored plane m = 0 /
-  // nz-1 with phi even, the advective flux phi u odd in every component (no slip) and the
-  // sharpening flux odd in its wall-normal component only (neutral wetting).  In terms of the
-  // stored total flux Q = phi u + kappa phi (1-phi) n:
-  //   Qx(ghost) = Qx(m) - 2 phi(m) ux(m),  Qy likewise,  Qz(ghost) = -Qz(m),  phi(ghost) = phi(m),
-  // so the two ghost iterations of a column also read u of the wall plane.
+  // Walls (R19).  A ghost position (beyond a wall of any axis: the plane j = -1 / nz of the
+  // marching axis, a halo row beyond a y wall, a side column beyond an x wall) holds the mirrored
+  // node m with phi even, the advective flux phi u odd in every component once per wall crossed
+  // (no slip) and the sharpening flux odd in the components of the crossed axes only (neutral
+  // wetting).  In terms of the stored total flux Q = phi u + kappa phi (1-phi) n, with
+  // sa = (-1)^(walls crossed) and s_al = -1 if axis al was crossed, else +1:
+  //   Q_al(ghost) = s_al Q_al(m) + (sa - s_al) phi(m) u_al(m),      phi(ghost) = phi(m),
+  // so ghost positions also read u of the mirrored node (one wall on z: Qx - 2 phi ux, Qy - 2 phi
+  // uy, -Qz).
   auto zsrc = [&](int j) {
     if (j < 0) return P.bcz ? -1 - j : j + P.nz;
     if (j >= P.nz) return P.bcz ? 2 * P.nz - 1 - j : j - P.nz;
     return j;
   };
   auto ghostify = [&](int j, T (&qx)[V], T (&qy)[V], T (&qz)[V], const T (&f)[V]) {
-    if (!(P.bcz && (j < 0 || j >= P.nz)) || !active) return;
+    const int kz = (P.bcz && (j < 0 || j >= P.nz)) ? 1 : 0;
+    if (!(kx | ky | kz) || !active) return;
+    const T sa = ((kx + ky + kz) & 1) ? T(-1) : T(1);
+    const T s0 = kx ? T(-1) : T(1), s1 = ky ? T(-1) : T(1), s2 = kz ? T(-1) : T(1);
     const long long s = col + (long long)plane * zsrc(j);
 #pragma unroll
     for (int i = 0; i < V; ++i) {
       if (xhalo && i > 0) break;
       T ux, uy, uz;
       load_u(S, P.N, s + i, ux, uy, uz);
-      qx[i] = fma(T(-2) * f[i], ux, qx[i]);
-      qy[i] = fma(T(-2) * f[i], uy, qy[i]);
-      qz[i] = -qz[i];
+      qx[i] = fma((sa - s0) * f[i], ux, s0 * qx[i]);
+      qy[i] = fma((sa - s1) * f[i], uy, s1 * qy[i]);
+      qz[i] = fma((sa - s2) * f[i], uz, s2 * qz[i]);
     }
   };
   auto issue = [&](int j, int slot) {              // one commit group per plane, possibly empty

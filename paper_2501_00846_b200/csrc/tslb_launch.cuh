@@ -206,12 +206,12 @@ inline int balanced_zchunk(long long tiles_xy, int nz, int slots) {
 
 // row kernel: V = 128 bit / sizeof(T) nodes per thread, 8 rows per block, cp.async 3 planes
 // ahead, planes per block chosen for whole waves (2 blocks per SM)
-template <typename T>
+template <typename T, bool WXY = false>
 cudaError_t launch_k1_row(const DevParams<T>& P, const T* S, const T* Q, T* D, cudaStream_t stream) {
   constexpr int TY = 8, MINB = 2, NSTAGE = 3;
   static_assert(TY + 2 <= 16, "one extra warp owns the 2 (TY + 2) side columns");
   constexpr int V = RowVec<T>::V;
-  auto kernel = k_allen_cahn_row<T, TY, MINB, NSTAGE>;
+  auto kernel = k_allen_cahn_row<T, TY, MINB, NSTAGE, WXY>;
   const size_t smem = sizeof(RowSmem<T, TY, NSTAGE>);
   static bool ready[kMaxDev] = {};
   cudaError_t e = prepare(kernel, smem, ready);
@@ -237,16 +237,17 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
   const bool forced = (flags & SEL_GENERIC) != 0;
   const bool row_ok = P.nx % RowVec<T>::V == 0;
   cudaError_t e;
-  // ---- K1 (interface tracking).  The flux-form kernels serve periodic tile axes; the row kernel
-  // also walls on the marching axis z (ghost flux planes).  Walls on x or y, where the two parts
-  // of the flux mirror differently, run the wall-capable kernel (normals recomputed on a ring of
-  // depth 2), which hands no flux over: K2 then writes none.
-  const bool k1_tiled = forced || side_walls || (P.bcz && !row_ok);
+  // ---- K1 (interface tracking).  The row kernel serves periodic axes and walls (ghost positions
+  // rebuild the mirrored flux from Q, phi and u); rows it cannot vectorise fall back to the
+  // one-node flux kernel on all-periodic boxes and to the wall-capable kernel (normals recomputed
+  // on a ring of depth 2) on boxes with walls, which hands no flux over: K2 then writes none.
+  const bool k1_tiled = forced || ((side_walls || P.bcz) && !row_ok);
   if (k1_tiled) {
     const bool walls = side_walls || P.bcz;
     e = walls ? launch_k1w<T, true>(P, S, D, stream) : launch_k1w<T, false>(P, S, D, stream);
-  } else if (row_ok && (P.bcz || !(flags & SEL_K1_FLUX))) {
-    e = launch_k1_row<T>(P, S, Q, D, stream);
+  } else if (row_ok && (side_walls || P.bcz || !(flags & SEL_K1_FLUX))) {
+    e = side_walls ? launch_k1_row<T, true>(P, S, Q, D, stream)
+                   : launch_k1_row<T, false>(P, S, Q, D, stream);
   } else {
     e = launch_k1_flux<T>(P, S, Q, D, stream);
   }

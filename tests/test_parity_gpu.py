@@ -226,10 +226,10 @@ def test_side_walls_on_the_lean_kernel(ref, bc, sel):
     the wall-adjacent receivers (wall_bounce) + the wall-capable interface kernel; the
     wall-capable pair is the cross-check.  Three x tiles, five y tiles, two z chunks, ragged;
     droplets sitting in a corner, on an edge and on a face, gravity oblique to every wall."""
-    shape = (40, 37, 70)                                         # (nz, ny, nx)
+    shape = (40, 37, 72)                                         # (nz, ny, nx); nx % 4 == 0: row kernel
     prm = I.base_params(bc=bc, body_accel=(1e-5, -2e-5, 1.5e-5))
     phi = I.sphere_profile(shape, (2.3, 1.8, 3.1), 7.0, 4.0, bc)            # low corner
-    phi += I.sphere_profile(shape, (67.2, 18.4, 37.6), 6.0, 4.0, bc)        # high x face / top
+    phi += I.sphere_profile(shape, (69.2, 18.4, 37.6), 6.0, 4.0, bc)        # high x face / top
     phi += I.sphere_profile(shape, (35.5, 35.1, 20.3), 5.0, 4.0, bc)        # high y face
     cfg = dict(name="side_walls", shape=shape, params=prm, phi=np.minimum(phi, 1.0),
                u=I.noise_u(shape, 1e-3, 59))
