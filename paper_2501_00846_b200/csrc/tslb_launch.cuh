@@ -270,10 +270,11 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
     const long long tiles = (long long)((P.nx + 31) / 32) * ((P.ny + 7) / 8);
     const bool deep = tiles * ((P.nz + 63) / 64) >= 3LL * 148 * minb;
     const int zc = deep ? 64 : balanced_zchunk(tiles, P.nz, 148 * minb);
-    // TMA tensor staging two planes ahead: fp64 production on deep grids with full tile rows
-    // (0.79 ms on 256^3 against 0.85 ms with cp.async); elsewhere only when asked for
+    // TMA tensor staging two planes ahead: fp64 production wherever the tile rows are full
+    // (256^3: 0.79 against 0.85 ms with cp.async; 192^3, 128^3, 96^3, 64^3: +10, +8, +5, +4 % in
+    // GLUPS); in fp32 (two blocks per SM) only when asked for (it loses 4 %)
     bool want_tma = tc && tma_usable(P) && !side_walls && !(flags & SEL_K2_CPASYNC) &&
-                    ((flags & SEL_K2_TMA) || (sizeof(T) == 8 && deep));
+                    ((flags & SEL_K2_TMA) || sizeof(T) == 8);
     e = cudaErrorNotSupported;
     if (want_tma) e = launch_tma<T, 8, minb, 2>(P, S, D, Qk2, stream, zc, tc);
     if (e == cudaErrorNotSupported) {          // not wanted, or no tensor-map encoder: cp.async
