@@ -280,12 +280,11 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
     if (e == cudaErrorNotSupported) {          // not wanted, or no tensor-map encoder: cp.async
       if (side_walls) {
         if constexpr (sizeof(T) == 8) e = launch_fast<T, 8, 1, 1, true>(P, S, D, Qk2, stream, zc);
-        else e = launch_fast<T, 8, 2, 1, true>(P, S, D, Qk2, stream, zc);
+        else e = launch_fast<T, 8, 2, 2, true>(P, S, D, Qk2, stream, zc);
       } else if constexpr (sizeof(T) == 8) {
         e = launch_fast<T, 8, 1, 1>(P, S, D, Qk2, stream, zc);
-      } else {
-        e = deep ? launch_fast<T, 8, 2, 2>(P, S, D, Qk2, stream, zc)
-                 : launch_fast<T, 8, 2, 1>(P, S, D, Qk2, stream, zc);
+      } else {      // fp32: two planes ahead on every grid (one ahead: -9 % at 128^3 / 192^3)
+        e = launch_fast<T, 8, 2, 2>(P, S, D, Qk2, stream, zc);
       }
     }
   }
