@@ -44,13 +44,15 @@ enum { TSLB_OK = 0, TSLB_EINVAL = -1, TSLB_EWORKSPACE = -2, TSLB_ECUDA = -3, TSL
  * makes tslb_create fail with TSLB_EINVAL. */
 enum {
   TSLB_FLAG_NAIVE = 1,      /* one-thread-per-node global-memory kernels (validation path)        */
-  TSLB_FLAG_GENERIC = 2,    /* on an all-periodic box, the wall-capable tiled pair                */
-  TSLB_FLAG_K2_CPASYNC = 4, /* lean periodic stream-collide kernel with cp.async staging, even
-                               where the TMA-staged one would be chosen                           */
+  TSLB_FLAG_GENERIC = 2,    /* the wall-capable tiled pair (explicit populations, normals
+                               recomputed) instead of the lean pair, on any box                  */
+  TSLB_FLAG_K2_CPASYNC = 4, /* lean stream-collide kernel with cp.async staging, even where the
+                               TMA-staged one would be chosen                                    */
   TSLB_FLAG_K2_TMA = 8,     /* ... with TMA tensor staging wherever it is usable (nx % 32 == 0,
-                               nx >= 64, ny > 8), even where cp.async would be chosen            */
-  TSLB_FLAG_K1_FLUX = 16,   /* one-node-per-thread flux-form interface kernel instead of the row
-                               kernel                                                             */
+                               nx >= 64, ny > 8, periodic x and y), even where cp.async would be
+                               chosen                                                            */
+  TSLB_FLAG_K1_FLUX = 16,   /* on an all-periodic box, the one-node-per-thread flux-form interface
+                               kernel instead of the row kernel                                  */
   TSLB_FLAG_ALL = 31
 };
 
