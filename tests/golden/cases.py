@@ -27,6 +27,11 @@ CASES = {
     "bubble128x128x256": (lambda: I.rising_bubble(), [1, 10, 100, 200, 300, 400, 500]),
     # ---- configs[3]: head-on collision at the graded 256^3
     "collision256": (lambda: I.head_on_collision(n=256), [1, 10, 50, 100, 200, 500, 1000]),
+    # ---- configs[3] and [4] at HALF size for their full nominal step counts (5000 / 1000);
+    # the emulsion keeps its volume fraction (200 droplets / 8)
+    "collision128": (lambda: I.head_on_collision(n=128, radius=12.0, half_sep=20.0),
+                     [1, 10, 100, 1000, 2000, 3000, 4000, 5000]),
+    "emulsion192": (lambda: I.emulsion_sweep(n=192, n_drops=25), [1, 10, 100, 500, 1000]),
     # ---- configs[4]: emulsion at 384^3 (the oracle needs ~40 GB there; 512^3 does not fit)
     "emulsion384": (lambda: I.emulsion_sweep(n=384), [1, 5, 10, 20, 50]),
     # ---- NEXT-2: off-axis collision, impact parameter 0.4, at 128^3
