@@ -37,8 +37,8 @@ FLOP_PER_UPDATE = 900.0                 # 0.8-1.0 kflop with eve
 # dram__bytes_read.sum + dram__bytes_write.sum per STEP (all kernels of one step) on the 256^3
 # collision workload, copied from the ncu --set full captures named beside them (not measured by
 # this run: ncu cannot run inside a timed bench)
-NCU_TRAFFIC = {"f64": (1.976867e9 + 2.103060e9 + 0.562707e9 + 0.122309e9, "profiles/r2_kernels_f64.txt"),
-               "f32": (0.977179e9 + 1.029355e9 + 0.285364e9 + 0.051619e9, "profiles/r2_kernels_f32.txt")}
+NCU_TRAFFIC = {"f64": (1.980335e9 + 2.102991e9 + 0.563100e9 + 0.118991e9, "profiles/r2_kernels_f64.txt"),
+               "f32": (0.977072e9 + 1.029373e9 + 0.285394e9 + 0.050653e9, "profiles/r2_kernels_f32.txt")}
 
 
 def parse():
