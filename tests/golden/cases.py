@@ -15,7 +15,7 @@ CASES = {
     "collision64": (lambda: I.head_on_collision(n=64, radius=6.0, half_sep=10.0),
                     [1, 10, 100, 1000, 1500]),
     "bubble32x32x64": (lambda: I.rising_bubble(nx=32, ny=32, nz=64, radius=6.0, height=16.0),
-                       [1, 10, 100, 1000, 2000]),
+                       [1, 10, 100, 1000, 2000, 5000, 10000, 20000]),
     # ---- configs[1]: Laplace sweep, 128^3, R in {12, 16, 24, 32}
     "laplace128_R12": (lambda: I.static_droplet(128, 12.0, seed=12), [1, 10, 100, 1000, 2000]),
     "laplace128_R16": (lambda: I.static_droplet(128, 16.0, seed=16), [1, 10, 100, 500, 1000]),

@@ -25,7 +25,7 @@ SEG = 10
 CASES = {
     "laplace128_R12": (lambda: I.static_droplet(128, 12.0, seed=12), [1000, 2000]),
     "bubble32x32x64": (lambda: I.rising_bubble(nx=32, ny=32, nz=64, radius=6.0, height=16.0),
-                       [1000, 2000]),
+                       [1000, 2000, 20000]),          # 20000 = configs[2]'s own step count
     "collision64": (lambda: I.head_on_collision(n=64, radius=6.0, half_sep=10.0), [1000, 1500]),
     "offaxis64": (lambda: I.off_axis_collision(n=64, impact=0.4), [600, 1200]),
 }
