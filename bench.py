@@ -34,6 +34,10 @@ METRIC = "GLUPS per B200 (fp32/fp64) and % of HBM roofline on 256^3 droplet doma
 STATE_SCALARS = 14                      # p*, u(3), Ahat(6), a(3), phi  -> 28 s bytes per update
 FLOP_PER_UPDATE = 900.0                 # 0.8-1.0 kflop with every node quantity
                                         # computed once (a1 70, a2 150, a4 100, a5 300, a6-a9 250)
+# flops actually EXECUTED per update (FMA = 2), from the instruction mix of the ncu captures in
+# profiles/r2_kernels_*.txt (K2 + K1, ring-cell redundancy included): the 0.9 kflop above is
+# SURVEY.md's estimate of the algorithm, this is what the kernels issue
+FLOP_EXECUTED = {"f64": 603.0, "f32": 615.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per STEP (all kernels of one step) on the 256^3
 # collision workload, copied from the ncu --set full captures named beside them (not measured by
 # this run: ncu cannot run inside a timed bench)
@@ -406,6 +410,8 @@ def roofline(r, prec, n, steps, peak, peak_kind, periodic_fast, full_size):
             "kernels": kernels,
             "alu_frac": alu_ach / r["fma_tflops"], "alu_achieved_tflops": alu_ach,
             "alu_peak_tflops": r["fma_tflops"], "alu_flop_per_update": FLOP_PER_UPDATE,
+            "alu_frac_executed": FLOP_EXECUTED[prec] * n / (ms_step * 1e-3) / 1e12 / r["fma_tflops"],
+            "alu_flop_per_update_executed": FLOP_EXECUTED[prec],
             "alu_peak_kind": "measured in this run (tslb_fma_peak, dependent-chain-free FMA)"}
 
 
