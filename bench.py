@@ -54,10 +54,11 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--size", type=int, default=256, help="cube edge of the domain")
     ap.add_argument("--workload", default="collision",
-                    choices=["collision", "emulsion", "bubble", "offaxis"],
+                    choices=["collision", "emulsion", "bubble", "offaxis", "train"],
                     help="collision = BASELINE.json configs[3] (the graded one); emulsion = "
                          "configs[4] (--size 384 for f64, 512 for f32); bubble = configs[2] "
-                         "(128x128x256, walls in z; --size scales it); offaxis = NEXT-2")
+                         "(128x128x256, walls in z; --size scales it); offaxis = NEXT-2; train = NEXT-2's "
+                         "droplet train falling onto a wall (128x128x768 at --size 256)")
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"],
                     help="precision of the headline value (the other one is reported beside it)")
     ap.add_argument("--flags", type=int, default=0,
@@ -154,6 +155,8 @@ def make_workload(size, kind="collision"):
         return cfg
     if kind == "offaxis":
         return I.off_axis_collision(n=size)
+    if kind == "train":                  # PAPER.md:354-366; box 1 : 1 : 6, walls in z
+        return I.droplet_train(nx=int(128 * s), ny=int(128 * s), nz=int(768 * s))
     return I.head_on_collision(n=size, radius=24.0 * s, half_sep=40.0 * s)
 
 

@@ -56,16 +56,26 @@ enum {
   TSLB_FLAG_ALL = 31
 };
 
+/* flags, second group: NOT a kernel selector but part of the problem statement.  The paper's
+ * body force acts "exclusively on the dispersed phase": the gas of a rising bubble (the
+ * default, force density (rho - rho_l) g, zero in the liquid) or the liquid of droplets falling
+ * through gas (force density (rho - rho_g) g, zero in the gas; reading R20b).
+ * Every kernel of the library honours it. */
+enum {
+  TSLB_FLAG_BODY_HEAVY = 32 /* body force (rho - rho_g) g : heavy (liquid) phase only             */
+};
+
 typedef struct tslb_params {
   double rho_l, rho_g;   /* > 0 ; rho = rho_g + phi (rho_l - rho_g)      */
   double mu_l, mu_g;     /* > 0 ; dynamic viscosities, mixed linearly in phi (R14) */
   double sigma;          /* >= 0 ; beta = 12 sigma/delta, kappa_mu = 3 sigma delta/2 P:136     */
   double delta;          /* > 0 ; interface width in lattice units */
   double mobility;       /* > 0 ; D of Eq. 4 ; kappa_AC = 4 D/delta    */
-  double body_accel[3];  /* g ; force density (rho - rho_l) g : light phase only    P:256, R20 */
+  double body_accel[3];  /* g ; force density (rho - rho_l) g : light phase only    P:256, R20 ;
+                            (rho - rho_g) g with TSLB_FLAG_BODY_HEAVY               P:358, R20b */
   int bc[3];             /* TSLB_BC_* for x, y, z                                              */
   int precision;         /* TSLB_F32 / TSLB_F64 : type of every field pointer and of all math  */
-  int flags;             /* TSLB_FLAG_* ; 0 for the production path                            */
+  int flags;             /* TSLB_FLAG_* ; 0 (or TSLB_FLAG_BODY_HEAVY alone) = production path   */
 } tslb_params;
 
 /* Bytes of device workspace tslb_create needs for this size and precision (0 on bad input). */

@@ -306,7 +306,7 @@ static void forces_at(const tslb_ref *h, const double *phi, int ix, int iy, int 
     for (int be = 0; be < 3; ++be)
       Fnu += Pineq[al][be] * (p->rho_l - p->rho_g) * gphi[be];
     Fnu *= -(nu * om / CS2);
-    double Fb = (rho - p->rho_l) * p->body_accel[al];                  /* R20 */
+    double Fb = (rho - (p->body_heavy ? p->rho_g : p->rho_l)) * p->body_accel[al];  /* R20, R20b */
     a[al] = (Fs + Fp + Fnu + Fb) / rho;                                /* R5  */
   }
 }

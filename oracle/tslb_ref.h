@@ -39,6 +39,8 @@ typedef struct tslb_ref_params {
   double mobility;       /* D of Eq. 4; kappa_AC = 4 D/delta */
   double body_accel[3];  /* g ; force density (rho - rho_l) g            PAPER.md:256, R20 */
   int bc[3];             /* TSLB_REF_PERIODIC / TSLB_REF_WALL per axis */
+  int body_heavy;        /* 0: force density (rho - rho_l) g ; 1: (rho - rho_g) g, the
+                            dispersed phase being the liquid            PAPER.md:358, R20b */
 } tslb_ref_params;
 
 typedef struct tslb_ref tslb_ref;

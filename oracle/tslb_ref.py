@@ -48,16 +48,18 @@ class Params(C.Structure):
     _fields_ = [("rho_l", C.c_double), ("rho_g", C.c_double),
                 ("mu_l", C.c_double), ("mu_g", C.c_double),
                 ("sigma", C.c_double), ("delta", C.c_double), ("mobility", C.c_double),
-                ("body_accel", C.c_double * 3), ("bc", C.c_int * 3)]
+                ("body_accel", C.c_double * 3), ("bc", C.c_int * 3),
+                ("body_heavy", C.c_int)]
 
 
 def make_params(rho_l, rho_g, mu_l, mu_g, sigma, delta, mobility,
-                body_accel=(0.0, 0.0, 0.0), bc=(0, 0, 0)):
+                body_accel=(0.0, 0.0, 0.0), bc=(0, 0, 0), body_heavy=False):
     p = Params()
     p.rho_l, p.rho_g, p.mu_l, p.mu_g = rho_l, rho_g, mu_l, mu_g
     p.sigma, p.delta, p.mobility = sigma, delta, mobility
     p.body_accel[:] = [float(v) for v in body_accel]
     p.bc[:] = [int(v) for v in bc]
+    p.body_heavy = 1 if body_heavy else 0
     return p
 
 

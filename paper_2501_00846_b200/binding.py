@@ -14,6 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libtslb.so")
 BC_PERIODIC, BC_WALL = 0, 1
 F32, F64 = 0, 1
 FLAG_NAIVE, FLAG_GENERIC, FLAG_K2_CPASYNC, FLAG_K2_TMA, FLAG_K1_FLUX = 1, 2, 4, 8, 16
+FLAG_BODY_HEAVY = 32        # body force (rho - rho_g) g instead of (rho - rho_l) g
 NDIAG = 16
 DIAG_NAMES = ("sum_phi", "sum_pstar", "max_u", "sum_phi_x", "sum_phi_y", "sum_phi_z",
               "sum_phi_ux", "sum_phi_uy", "sum_phi_uz", "sum_ux", "sum_uy", "sum_uz",
@@ -35,13 +36,14 @@ class tslb_params(C.Structure):
 
 
 def make_params(rho_l, rho_g, mu_l, mu_g, sigma, delta, mobility, body_accel=(0.0, 0.0, 0.0),
-                bc=(0, 0, 0), precision=F64, flags=0):
+                bc=(0, 0, 0), precision=F64, flags=0, body_heavy=False):
     p = tslb_params()
     p.rho_l, p.rho_g, p.mu_l, p.mu_g = rho_l, rho_g, mu_l, mu_g
     p.sigma, p.delta, p.mobility = sigma, delta, mobility
     p.body_accel[:] = [float(v) for v in body_accel]
     p.bc[:] = [int(v) for v in bc]
-    p.precision, p.flags = int(precision), int(flags)
+    p.precision = int(precision)
+    p.flags = int(flags) | (FLAG_BODY_HEAVY if body_heavy else 0)
     return p
 
 

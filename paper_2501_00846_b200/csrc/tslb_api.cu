@@ -40,7 +40,7 @@ bool params_ok(int nx, int ny, int nz, const tslb_params* p) {
         p->mobility > 0 && p->sigma >= 0))
     return false;
   if (p->precision != TSLB_F32 && p->precision != TSLB_F64) return false;
-  if (p->flags & ~TSLB_FLAG_ALL) return false;   // stray bits never select anything
+  if (p->flags & ~(TSLB_FLAG_ALL | TSLB_FLAG_BODY_HEAVY)) return false;   // stray bits never select anything
   const int n[3] = {nx, ny, nz};
   for (int d = 0; d < 3; ++d) {
     if (p->bc[d] != TSLB_BC_PERIODIC && p->bc[d] != TSLB_BC_WALL) return false;
@@ -65,6 +65,7 @@ tslb::DevParams<T> make_dev(int nx, int ny, int nz, const tslb_params& p, long l
   d.bcx = p.bc[0]; d.bcy = p.bc[1]; d.bcz = p.bc[2];
   d.N = stride;
   d.rho_l = T(p.rho_l); d.rho_g = T(p.rho_g); d.drho = T(p.rho_l - p.rho_g);
+  d.rho_b = (p.flags & TSLB_FLAG_BODY_HEAVY) ? d.rho_g : d.rho_l;
   d.mu_g = T(p.mu_g); d.dmu = T(p.mu_l - p.mu_g);
   d.beta4 = T(4.0 * 12.0 * p.sigma / p.delta);
   d.kappa_mu = T(3.0 * p.sigma * p.delta / 2.0);

@@ -100,6 +100,7 @@ struct DevParams {
                               // flux-form interface kernels (the centre weight 1 - 216 c2 is never
                               // formed: the kernels add an increment of differences to phi)
   T gx, gy, gz;               // body acceleration                          (R20)
+  T rho_b;                    // force density (rho - rho_b) g: rho_l or rho_g (R20b)
 };
 
 template <typename T> __device__ __forceinline__ T rsqrt_t(T x);
@@ -219,14 +220,14 @@ __device__ __forceinline__ NodeOut<T> close_node(const DevParams<T>& P, const Mo
   T pc = m.p * cs2;
   T nxx = m.xx - pc - uox * uox, nyy = m.yy - pc - uoy * uoy, nzz = m.zz - pc - uoz * uoz;
   T nxy = m.xy - uox * uoy, nxz = m.xz - uox * uoz, nyz = m.yz - uoy * uoz;
-  // F = mu_phi grad(phi) - p* cs^2 grad(rho) - (nu omega/cs^2) Pi^neq . grad(rho) + (rho - rho_l) g
-  // with grad(rho) = drho grad(phi) (R18):  F = k1 grad(phi) - k2 Pi^neq.grad(phi) + (rho-rho_l) g
+  // F = mu_phi grad(phi) - p* cs^2 grad(rho) - (nu omega/cs^2) Pi^neq . grad(rho) + (rho - rho_b) g
+  // with grad(rho) = drho grad(phi) (R18):  F = k1 grad(phi) - k2 Pi^neq.grad(phi) + (rho-rho_b) g
   T k1 = mu_phi - pc * P.drho;
   T k2 = mx.nuom3 * P.drho;
   T fx = k1 * gx - k2 * (nxx * gx + nxy * gy + nxz * gz);
   T fy = k1 * gy - k2 * (nxy * gx + nyy * gy + nyz * gz);
   T fz = k1 * gz - k2 * (nxz * gx + nyz * gy + nzz * gz);
-  T db = mx.rho - P.rho_l;
+  T db = mx.rho - P.rho_b;
   NodeOut<T> o;
   o.ax = fma(db, P.gx, fx) * mx.inv_rho;
   o.ay = fma(db, P.gy, fy) * mx.inv_rho;

@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(256) k_init(DevParams<T> P, long long nodes,
   T ph = phi0[idx];
   Mix<T> mx = mixture(P, ph);
   T mu_phi = P.beta4 * ph * (ph - T(1)) * (ph - T(0.5)) - P.kappa_mu * lap;
-  T db = mx.rho - P.rho_l;
+  T db = mx.rho - P.rho_b;
   NodeOut<T> o = {};
   o.ux = u0[idx]; o.uy = u0[us + idx]; o.uz = u0[2 * us + idx];
   o.ax = fma(db, P.gx, mu_phi * gx) * mx.inv_rho;

@@ -223,6 +223,42 @@ def off_axis_collision(n=256, impact=0.38, weber=53.0, radius=None, half_sep=Non
                 phi=phi1 + phi2, u=u)
 
 
+def droplet_train(nx=128, ny=128, nz=768, n_drops=5, spacing=2.0, weber=40.0, speed=0.05,
+                  bond=1.0, seed=6, noise=1e-6):
+    """SURVEY.md NEXT-2, second workload: a train of `n_drops` droplets falling
+    onto the bottom wall "under the effect of an initial velocity and the gravity"; periodic in x
+    and y, no-slip neutral-wetting walls at bottom and top (bc z = WALL: halfway bounce-back and
+    mirrored phi, R19), box 1 : 1 : 6 like the paper's 500 x 500 x 3000.  `spacing` = the paper's
+    Delta L in diameters (2 and 6 there), We = rho_l U^2 D / sigma = 40 with U = `speed` the impact
+    velocity.  Not given by the paper, chosen here: D = nx / 5; the lowest droplet starts 1.5 D
+    above the wall; Oh = 0.0044 as in its collision study with nu_l floored at 1/300
+    (tau_l >= 0.51, configs[3]'s value) so that reduced boxes stay inside the scheme's stable range;
+    g from a Bond number rho_l g D^2 / sigma = `bond`, acting on the liquid (the dispersed phase
+    here: force density (rho - rho_g) g, TSLB_FLAG_BODY_HEAVY, R20b); rho ratio 800, mu
+    ratio 50 (configs[3])."""
+    shape = (nz, ny, nx)
+    D = nx / 5.0
+    radius = 0.5 * D
+    sigma = 1.0 * speed * speed * D / weber
+    reynolds = np.sqrt(weber) / 0.0044
+    mu_l = max(speed * D / reynolds, 1.0 / 300.0)
+    g = bond * sigma / (D * D)
+    prm = base_params(rho_g=1.0 / 800.0, sigma=sigma, mu_l=mu_l, mu_g=mu_l / 50.0,
+                      body_accel=(0.0, 0.0, -g), bc=(PERIODIC, PERIODIC, WALL), body_heavy=True)
+    top = 1.5 * D + (n_drops - 1) * spacing * D + radius
+    if top + 2.0 * prm["delta"] > nz - 1:
+        raise ValueError("droplet_train: %d droplets at spacing %g D do not fit nz = %d"
+                         % (n_drops, spacing, nz))
+    phi = np.zeros(shape)
+    for k in range(n_drops):
+        phi += sphere_profile(shape, ((nx - 1) / 2.0, (ny - 1) / 2.0, 1.5 * D + k * spacing * D),
+                              radius, prm["delta"], prm["bc"])
+    u = noise_u(shape, noise, seed) if noise else np.zeros((3,) + shape)
+    u[2] -= speed * phi
+    return dict(name=f"droplet_train_{nx}x{ny}x{nz}_dL{spacing:g}", shape=shape, params=prm,
+                phi=phi, u=u)
+
+
 def emulsion_sweep(n=384, n_drops=200, seed=5):
     """configs[4]: 200 droplets, radii in [6,14], solenoidal velocity of amplitude 0.02."""
     shape = (n, n, n)

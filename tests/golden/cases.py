@@ -36,4 +36,8 @@ CASES = {
     "emulsion384": (lambda: I.emulsion_sweep(n=384), [1, 5, 10, 20, 50]),
     # ---- NEXT-2: off-axis collision, impact parameter 0.4, at 128^3
     "offaxis128": (lambda: I.off_axis_collision(n=128, impact=0.4), [1, 10, 100, 300]),
+    # ---- NEXT-2, second workload: a train of 5 droplets falling onto the bottom
+    # wall (walls in z, gravity on the liquid, R20b); first contact near step 256, then every 512
+    "train64x64x192": (lambda: I.droplet_train(nx=64, ny=64, nz=192),
+                       [1, 10, 100, 300, 600, 1000, 1500]),
 }

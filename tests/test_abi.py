@@ -79,7 +79,7 @@ def test_create_argument_errors(B):
     for ok in (0, 1, 2, 4, 8, 16, 8 | 16):
         assert lib.tslb_create(32, 32, 32, C.byref(good(B, flags=ok)), fake, None, C.byref(h)) == 0
         lib.tslb_destroy(h)
-    for stray in (32, 1 << 8, 59 << 8, 1 << 16, 1 << 23):
+    for stray in (64, 1 << 8, 59 << 8, 1 << 16, 1 << 23):
         assert lib.tslb_create(32, 32, 32, C.byref(good(B, flags=stray)), fake, None,
                                C.byref(h)) == -1
     assert lib.tslb_step(None, 1) == -1

@@ -48,6 +48,38 @@ def test_p12_hydrostatic_rest_all_liquid(ref):
     assert np.all(phi == 1.0)
 
 
+def test_p12b_heavy_phase_body_force(ref):
+    """R20b (the droplet train "falling under ... the gravity"): with body_heavy
+    the force density is (rho - rho_g) g.  An all-gas box stays exactly at rest; an all-liquid
+    box accelerates uniformly at (rho_l - rho_g) g / rho_l, p* and A unchanged (the closed
+    form of P5 with the roles of the phases exchanged)."""
+    shape = (4, 4, 6)
+    sim, _ = make(ref, shape, np.zeros(shape), np.zeros((3,) + shape), body_accel=(0, 0, -1e-4),
+                  body_heavy=True)
+    sim.step(50)
+    ps, u, A, a, phi = sim.get_state()
+    assert np.abs(u).max() == 0.0 and np.abs(ps).max() == 0.0 and np.abs(a).max() == 0.0
+    g = np.array([1e-5, -2e-5, 3e-5])
+    sim, prm = make(ref, shape, np.ones(shape), np.zeros((3,) + shape), rho_g=0.25,
+                    body_accel=tuple(g), body_heavy=True)
+    acc = (prm["rho_l"] - prm["rho_g"]) * g / prm["rho_l"]
+    sim.step(100)
+    ps, u, A, a, _ = sim.get_state()
+    for al in range(3):
+        assert np.abs(u[al] - 100 * acc[al]).max() < 1e-15
+        assert np.abs(a[al] - acc[al]).max() < 1e-18
+    assert np.abs(ps).max() < 1e-16 and np.abs(A).max() < 1e-16
+    # and the default (R20) differs from it by exactly (rho_l - rho_g) g / rho at every node
+    phi0 = np.full(shape, 0.3)
+    s0, prm = make(ref, shape, phi0, np.zeros((3,) + shape), rho_g=0.25, body_accel=tuple(g))
+    s1, _ = make(ref, shape, phi0, np.zeros((3,) + shape), rho_g=0.25, body_accel=tuple(g),
+                 body_heavy=True)
+    rho = prm["rho_g"] + 0.3 * (prm["rho_l"] - prm["rho_g"])
+    a0, a1 = s0.get_state()[3], s1.get_state()[3]
+    for al in range(3):
+        assert np.abs((a1[al] - a0[al]) - (prm["rho_l"] - prm["rho_g"]) * g[al] / rho).max() < 1e-18
+
+
 # ---------------------------------------------------------------- P6 -------------------
 @pytest.mark.parametrize("nu", [0.005, 1.0 / 60.0, 0.2])
 def test_p6_shear_wave_decay(ref, nu):

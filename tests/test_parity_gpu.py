@@ -28,6 +28,15 @@ def _small_case(name):
         cfg = I.rising_bubble(nx=20, ny=12, nz=26, radius=5.0, height=9.0)
         cfg["u"] = I.noise_u(cfg["shape"], 1e-4, 22)
         return cfg, [1, 60]
+    elif name == "train_walls_z":            # NEXT-2 in miniature: droplets falling onto a wall,
+        shape = (30, 12, 20)                 # gravity on the LIQUID (R20b, TSLB_FLAG_BODY_HEAVY)
+        prm = I.base_params(rho_g=1.0 / 800.0, mu_l=1.0 / 300.0, mu_g=1.0 / 15000.0, sigma=8e-4,
+                            bc=(0, 0, 1), body_accel=(1e-6, 0.0, -2e-5), body_heavy=True)
+        phi = I.sphere_profile(shape, (9.6, 5.7, 5.2), 4.0, 4.0, prm["bc"])
+        phi += I.sphere_profile(shape, (9.6, 5.7, 17.3), 4.0, 4.0, prm["bc"])
+        u = I.noise_u(shape, 1e-4, 27)
+        u[2] -= 0.05 * phi
+        steps = [1, 60]
     elif name == "walls_all":                # droplet touching a corner, walls on every axis
         shape = (8, 9, 10)
         prm = I.base_params(bc=(1, 1, 1), body_accel=(1e-5, -2e-5, 3e-5))
@@ -84,8 +93,8 @@ def test_config0_static_droplet_fp32(ref, path):
 
 
 @pytest.mark.parametrize("path", PATHS)
-@pytest.mark.parametrize("case", ["ragged_periodic", "bubble_walls_z", "walls_all", "walls_xy",
-                                  "min_periodic", "min_walls"])
+@pytest.mark.parametrize("case", ["ragged_periodic", "bubble_walls_z", "train_walls_z", "walls_all",
+                                  "walls_xy", "min_periodic", "min_walls"])
 def test_small_cases_fp64(ref, path, case):
     cfg, steps = _small_case(case)
     want = run_oracle(ref, cfg, steps)
@@ -97,7 +106,7 @@ def test_small_cases_fp64(ref, path, case):
 
 
 @pytest.mark.parametrize("path", PATHS)
-@pytest.mark.parametrize("case", ["ragged_periodic", "bubble_walls_z", "walls_all"])
+@pytest.mark.parametrize("case", ["ragged_periodic", "bubble_walls_z", "train_walls_z", "walls_all"])
 def test_small_cases_fp32(ref, path, case):
     cfg, steps = _small_case(case)
     want = run_oracle(ref, cfg, steps)
@@ -236,10 +245,23 @@ def test_side_walls_on_the_lean_kernel(ref, bc, sel):
     _check_both_precisions(ref, cfg, [1, 2, 12], SELECTORS[sel], f"side walls {bc}/{sel}")
 
 
+@pytest.mark.parametrize("sel", ["generic", "k2_cpasync"])
+def test_heavy_phase_body_force_on_every_pair(ref, sel):
+    """R20b: the body-force reference density is part of the problem, not of a kernel: the
+    wall-capable pair and the lean pair give the oracle's fields with it too, and the fields
+    differ from the default R20 run (so the bit cannot be silently dropped)."""
+    cfg, steps = _small_case("train_walls_z")
+    _check_both_precisions(ref, cfg, steps, SELECTORS[sel], f"train/{sel}")
+    other = dict(cfg, params=dict(cfg["params"], body_heavy=False))
+    a, _ = run_gpu(cfg, [10], "f64", SELECTORS[sel])
+    b, _ = run_gpu(other, [10], "f64", SELECTORS[sel])
+    assert rel_err(a[0]["u"], b[0]["u"]) > 1e-3
+
+
 def test_stray_flag_bits_are_rejected():
     from paper_2501_00846_b200 import binding as B
     cfg = I.static_droplet(16, 4.0, seed=2)
-    for flags in (32, 1 << 8, 59 << 8, 1 << 16, 1 << 30):
+    for flags in (64, 1 << 8, 59 << 8, 1 << 16, 1 << 30):
         with pytest.raises(B.TslbError):
             B.Solver(16, 16, 16, cfg["params"], flags=flags)
 
