@@ -65,6 +65,10 @@ def parse():
                     help="validation selector (include/tslb.h TSLB_FLAG_*), 0 = production")
     ap.add_argument("--bc", default=None,
                     help="override the boundary types, e.g. 1,1,1 = walls on x, y and z")
+    ap.add_argument("--slab-overlap", default="auto", choices=["auto", "on", "off"],
+                    help="--decomp slab: compute and send the face planes first and sweep the "
+                         "interior while they travel (tslb_slab_step_faces / _interior); auto = "
+                         "on when there is a transfer to hide (N > 1)")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (weak scaling; BASELINE.json's north star, "
                          "the default) or ONE lattice cut into z slabs with a halo exchange per "
@@ -290,7 +294,8 @@ def measure_slab(cfg, precision, args, device, ranks):
     sl.init(cfg["phi"], cfg["u"])
     sl.exchange()
     d0 = sl.solver.diag()
-    sl.step(args.warmup)
+    overlap = args.slab_overlap == "on" or (args.slab_overlap == "auto" and ranks.world > 1)
+    sl.step(args.warmup, overlap=overlap)
     torch.cuda.synchronize(device)
     sampler = ClockSampler(torch.device(device).index or 0)
     sampler.start()
@@ -301,7 +306,7 @@ def measure_slab(cfg, precision, args, device, ranks):
         torch.cuda.synchronize(device)
         ranks.barrier()
         e0.record(sl.solver.stream)
-        sl.step(args.steps)
+        sl.step(args.steps, overlap=overlap)
         e1.record(sl.solver.stream)
         torch.cuda.synchronize(device)
         ranks.barrier()
@@ -475,8 +480,11 @@ def main():
                 "scaling": "strong" if slab else "weak", "vs_baseline": None, "dtype": order[0],
                 "data": "synthetic",
                 "config": {"workload": cfg["name"], "grid": list(cfg["shape"][::-1]),
-                           "parallelism": (f"z-slabs x{world}, halo exchange per step" if slab
-                                           else f"replicas x{world}"),
+                           "parallelism": (f"z-slabs x{world}, halo exchange per step"
+                                           + (", overlapped with the interior sweep"
+                                              if args.slab_overlap == "on" or
+                                              (args.slab_overlap == "auto" and world > 1) else "")
+                                           if slab else f"replicas x{world}"),
                            "l2": f"state {2 * STATE_SCALARS * es0 * n / 1e9:.1f} GB ({order[0]}) >> 126 MB L2: "
                                  "inputs larger than L2, no flush needed",
                            "flags": args.flags,

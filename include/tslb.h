@@ -138,6 +138,21 @@ size_t tslb_halo_bytes(const tslb_handle *h);
 int tslb_halo_pack(tslb_handle *h, int face, void *buf);
 int tslb_halo_unpack(tslb_handle *h, int face, const void *buf);
 
+/* The same step of a slab in two stages, so that the exchange overlaps the interior sweep
+ * (the paper's decompositions and their communication cost: P:194-238):
+ *   tslb_slab_step_faces(h):    interface update (Eq. 20) on planes [1, nz-1), stream-collide on
+ *                               the owned planes next to the faces, [2, 4) and [nz-4, nz-2); the
+ *                               state buffers swap, so tslb_halo_pack now packs the NEW faces;
+ *   tslb_slab_step_interior(h): stream-collide on the interior [4, nz-4): the step is complete.
+ * Between the two only tslb_halo_pack / tslb_halo_unpack may be called (anything else returns
+ * TSLB_ESTATE): pack, start the transfer, run the interior, wait, unpack.  The ghost planes are
+ * never computed (the exchange fills them), so the owned planes come out bit-identical to
+ * tslb_step(1) + exchange and to the undivided lattice.  Requirements of tslb_halo_pack, and nx
+ * a multiple of the 128-bit vector width (2 in fp64, 4 in fp32).  Three or four launches on the
+ * handle's stream, no synchronisation. */
+int tslb_slab_step_faces(tslb_handle *h);
+int tslb_slab_step_interior(tslb_handle *h);
+
 /* On-device diagnostics: box reductions of the current state, the
  * quantities behind the paper's validation plots (centre-of-mass velocity of a rising bubble,
  * Fig. 4) and BASELINE.json's checks (sum(phi) conserved; Laplace's law

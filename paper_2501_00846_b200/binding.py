@@ -24,6 +24,7 @@ SYMBOLS = ("tslb_workspace_bytes", "tslb_create", "tslb_init", "tslb_step", "tsl
            "tslb_get_state", "tslb_set_state", "tslb_init_host", "tslb_get_host", "tslb_step_timed",
            "tslb_launch_count", "tslb_diag", "tslb_diag_host", "tslb_diag_static", "tslb_fma_peak",
            "tslb_halo_bytes", "tslb_halo_pack", "tslb_halo_unpack",
+           "tslb_slab_step_faces", "tslb_slab_step_interior",
            "tslb_destroy", "tslb_last_error")
 
 
@@ -80,6 +81,8 @@ def load():
     lib.tslb_halo_bytes.restype = C.c_size_t
     lib.tslb_halo_pack.argtypes = [vp, C.c_int, vp]
     lib.tslb_halo_unpack.argtypes = [vp, C.c_int, vp]
+    lib.tslb_slab_step_faces.argtypes = [vp]
+    lib.tslb_slab_step_interior.argtypes = [vp]
     lib.tslb_launch_count.argtypes = [vp]
     lib.tslb_launch_count.restype = C.c_longlong
     lib.tslb_destroy.argtypes = [vp]
@@ -217,6 +220,13 @@ class Solver:
 
     def halo_unpack(self, face, buf):
         self._call("tslb_halo_unpack", int(face), buf.data_ptr())
+
+    def slab_step_faces(self):
+        """First stage of a slab's step: afterwards halo_pack packs the NEW face planes."""
+        self._call("tslb_slab_step_faces")
+
+    def slab_step_interior(self):
+        self._call("tslb_slab_step_interior")
 
     def diag(self):
         """tslb_diag_host: dict of the TSLB_D_* box reductions (synchronises the stream)."""

@@ -63,6 +63,7 @@ tslb::DevParams<T> make_dev(int nx, int ny, int nz, const tslb_params& p, long l
   tslb::DevParams<T> d;
   d.nx = nx; d.ny = ny; d.nz = nz;
   d.bcx = p.bc[0]; d.bcy = p.bc[1]; d.bcz = p.bc[2];
+  d.zbeg = 0; d.zend = nz;
   d.N = stride;
   d.rho_l = T(p.rho_l); d.rho_g = T(p.rho_g); d.drho = T(p.rho_l - p.rho_g);
   d.rho_b = (p.flags & TSLB_FLAG_BODY_HEAVY) ? d.rho_g : d.rho_l;
@@ -90,6 +91,7 @@ struct tslb_handle {
   double* diag;          // diag_rows(nodes) + 1 rows of NDIAG doubles (tslb_diag partial sums)
   int cur;
   bool inited;
+  bool split;            // between tslb_slab_step_faces and tslb_slab_step_interior
   long long launches;
   tslb::TmaCache tma;     // tensor maps of the two state buffers (TMA-staged kernel)
 };
@@ -127,6 +129,7 @@ int tslb_create(int nx, int ny, int nz, const tslb_params* p, void* workspace, v
   h->diag = reinterpret_cast<double*>(w + pb * size_t(2 * tslb::NFIELD + scratch_planes(p)));
   h->cur = 0;
   h->inited = false;
+  h->split = false;
   h->launches = 0;
   *out = h;
   return TSLB_OK;
@@ -146,6 +149,7 @@ int init_impl(tslb_handle* h, const T* phi, const T* u, long long u_stride) {
   auto P = make_dev<T>(h->nx, h->ny, h->nz, h->prm, h->stride);
   T* D = reinterpret_cast<T*>(h->buf[0]);
   h->cur = 0;
+  h->split = false;
   unsigned blocks = unsigned((h->nodes + 255) / 256);
   tslb::k_init<T><<<blocks, 256, 0, h->stream>>>(P, h->nodes, phi, u, u_stride, D,
                                                  reinterpret_cast<T*>(h->scratch));
@@ -180,6 +184,43 @@ int step_impl(tslb_handle* h, int n, const tslb::Marker& mk) {
     h->cur ^= 1;
   }
   CUDA_TRY(cudaGetLastError());
+  return TSLB_OK;
+}
+
+// The step of a z-slab (two ghost planes per end, include/tslb.h) in two stages, so that the
+// exchange of the freshly computed face planes can travel while the interior is still being
+// computed.  Stage 0: interface update on planes [1, nz-1) (everything the owned planes' forces
+// read), stream-collide on the owned planes next to the faces, [2, 4) and [nz-4, nz-2); the
+// buffers swap, so tslb_halo_pack sees the new faces.  Stage 1: stream-collide on the interior
+// [4, nz-4).  The ghost planes are not computed at all: the exchange fills them.
+template <typename T>
+int slab_step_impl(tslb_handle* h, int stage) {
+  auto P = make_dev<T>(h->nx, h->ny, h->nz, h->prm, h->stride);
+  const int g = tslb::HALO_DEPTH, nz = h->nz;
+  const int lo_end = std::min(2 * g, nz - g), hi_beg = std::max(nz - 2 * g, lo_end);
+  const T* S = reinterpret_cast<const T*>(h->buf[stage == 0 ? h->cur : h->cur ^ 1]);
+  T* D = reinterpret_cast<T*>(h->buf[stage == 0 ? h->cur ^ 1 : h->cur]);
+  T* Q = reinterpret_cast<T*>(h->scratch);
+  cudaError_t e = cudaSuccess;
+  auto k2 = [&](int zb, int ze) {
+    if (e != cudaSuccess || ze <= zb) return;
+    P.zbeg = zb; P.zend = ze;
+    e = tslb::launch_k2_stage<T>(P, S, D, Q, h->stream, h->prm.flags, &h->tma);
+    h->launches += 1;
+  };
+  if (stage == 0) {
+    P.zbeg = 1; P.zend = nz - 1;
+    e = tslb::launch_k1_stage<T>(P, S, D, Q, h->stream, h->prm.flags);
+    h->launches += 1;
+    k2(g, lo_end);
+    k2(hi_beg, nz - g);
+    h->cur ^= 1;
+    h->split = true;
+  } else {
+    k2(lo_end, hi_beg);
+    h->split = false;
+  }
+  if (e != cudaSuccess) return fail(TSLB_ECUDA, "slab step: %s", cudaGetErrorString(e));
   return TSLB_OK;
 }
 
@@ -268,6 +309,7 @@ int tslb_init(tslb_handle* h, const void* phi, const void* u) {
 int tslb_step(tslb_handle* h, int n) {
   if (!h || n < 0) return fail(TSLB_EINVAL, "tslb_step: NULL handle or n < 0");
   if (!h->inited) return fail(TSLB_ESTATE, "tslb_step before tslb_init");
+  if (h->split) return fail(TSLB_ESTATE, "tslb_step between tslb_slab_step_faces and tslb_slab_step_interior");
   tslb::Marker none;
   return h->prm.precision == TSLB_F64 ? step_impl<double>(h, n, none)
                                       : step_impl<float>(h, n, none);
@@ -276,6 +318,7 @@ int tslb_step(tslb_handle* h, int n) {
 int tslb_step_timed(tslb_handle* h, int n, float* kernel_ms) {
   if (!h || n < 0 || !kernel_ms) return fail(TSLB_EINVAL, "tslb_step_timed: bad argument");
   if (!h->inited) return fail(TSLB_ESTATE, "tslb_step_timed before tslb_init");
+  if (h->split) return fail(TSLB_ESTATE, "tslb_step_timed between tslb_slab_step_faces and tslb_slab_step_interior");
   std::vector<cudaEvent_t> ev;
   std::vector<int> kind;
   tslb::Marker mk;
@@ -297,6 +340,7 @@ int tslb_step_timed(tslb_handle* h, int n, float* kernel_ms) {
 int tslb_get(tslb_handle* h, void* rho, void* p, void* u, void* phi) {
   if (!h) return fail(TSLB_EINVAL, "tslb_get: NULL handle");
   if (!h->inited) return fail(TSLB_ESTATE, "tslb_get before tslb_init");
+  if (h->split) return fail(TSLB_ESTATE, "tslb_get between tslb_slab_step_faces and tslb_slab_step_interior");
   if (h->prm.precision == TSLB_F64)
     return get_impl<double>(h, (double*)rho, (double*)p, (double*)u, h->nodes, (double*)phi);
   return get_impl<float>(h, (float*)rho, (float*)p, (float*)u, h->nodes, (float*)phi);
@@ -305,6 +349,7 @@ int tslb_get(tslb_handle* h, void* rho, void* p, void* u, void* phi) {
 int tslb_get_state(tslb_handle* h, void* pstar, void* u, void* A, void* a, void* phi) {
   if (!h) return fail(TSLB_EINVAL, "tslb_get_state: NULL handle");
   if (!h->inited) return fail(TSLB_ESTATE, "tslb_get_state before tslb_init");
+  if (h->split) return fail(TSLB_ESTATE, "tslb_get_state between tslb_slab_step_faces and tslb_slab_step_interior");
   unsigned blocks = unsigned((h->nodes + 255) / 256);
   if (h->prm.precision == TSLB_F64) {
     auto P = make_dev<double>(h->nx, h->ny, h->nz, h->prm, h->stride);
@@ -327,6 +372,7 @@ int tslb_set_state(tslb_handle* h, const void* pstar, const void* u, const void*
   if (!h || !pstar || !u || !A || !a || !phi) return fail(TSLB_EINVAL, "tslb_set_state: NULL argument");
   unsigned blocks = unsigned((h->nodes + 255) / 256);
   h->cur = 0;
+  h->split = false;
   if (h->prm.precision == TSLB_F64) {
     auto P = make_dev<double>(h->nx, h->ny, h->nz, h->prm, h->stride);
     tslb::k_set_state<double><<<blocks, 256, 0, h->stream>>>(
@@ -376,6 +422,34 @@ int tslb_halo_unpack(tslb_handle* h, int face, const void* buf) {
                                       : halo_launch<float, false>(h, face, const_cast<void*>(buf));
 }
 
+static int slab_step_check(const tslb_handle* h, const char* who) {
+  if (!h) return fail(TSLB_EINVAL, "%s: NULL handle", who);
+  if (!h->inited) return fail(TSLB_ESTATE, "%s before tslb_init", who);
+  if (h->prm.bc[2] != TSLB_BC_PERIODIC || h->nz < 3 * tslb::HALO_DEPTH ||
+      h->prm.bc[0] != TSLB_BC_PERIODIC || h->prm.bc[1] != TSLB_BC_PERIODIC ||
+      (h->prm.flags & (TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC)))
+    return fail(TSLB_EINVAL, "%s: needs what tslb_halo_pack needs (periodic box, >= 6 planes, lean pair)", who);
+  const int vec = h->prm.precision == TSLB_F64 ? 2 : 4;
+  if (h->nx % vec != 0)
+    return fail(TSLB_EINVAL, "%s: nx must be a multiple of %s (the row kernel of the interface update)", who,
+                vec == 2 ? "2" : "4");
+  return TSLB_OK;
+}
+
+int tslb_slab_step_faces(tslb_handle* h) {
+  int rc = slab_step_check(h, "tslb_slab_step_faces");
+  if (rc != TSLB_OK) return rc;
+  if (h->split) return fail(TSLB_ESTATE, "tslb_slab_step_faces twice without tslb_slab_step_interior");
+  return h->prm.precision == TSLB_F64 ? slab_step_impl<double>(h, 0) : slab_step_impl<float>(h, 0);
+}
+
+int tslb_slab_step_interior(tslb_handle* h) {
+  int rc = slab_step_check(h, "tslb_slab_step_interior");
+  if (rc != TSLB_OK) return rc;
+  if (!h->split) return fail(TSLB_ESTATE, "tslb_slab_step_interior without tslb_slab_step_faces");
+  return h->prm.precision == TSLB_F64 ? slab_step_impl<double>(h, 1) : slab_step_impl<float>(h, 1);
+}
+
 // partial sums into `rows` (device scratch of diag_rows(nodes) rows), result into `out` (device)
 static int diag_launch(tslb_handle* h, double* rows, double* out) {
   const unsigned blocks = unsigned(tslb::diag_rows(h->nodes));
@@ -397,12 +471,14 @@ static int diag_launch(tslb_handle* h, double* rows, double* out) {
 int tslb_diag(tslb_handle* h, double* out) {
   if (!h || !out) return fail(TSLB_EINVAL, "tslb_diag: NULL argument");
   if (!h->inited) return fail(TSLB_ESTATE, "tslb_diag before tslb_init");
+  if (h->split) return fail(TSLB_ESTATE, "tslb_diag between tslb_slab_step_faces and tslb_slab_step_interior");
   return diag_launch(h, h->diag, out);
 }
 
 int tslb_diag_host(tslb_handle* h, double* out) {
   if (!h || !out) return fail(TSLB_EINVAL, "tslb_diag_host: NULL argument");
   if (!h->inited) return fail(TSLB_ESTATE, "tslb_diag_host before tslb_init");
+  if (h->split) return fail(TSLB_ESTATE, "tslb_diag_host between tslb_slab_step_faces and tslb_slab_step_interior");
   double* d_out = h->diag + tslb::diag_rows(h->nodes) * tslb::NDIAG;
   int rc = diag_launch(h, h->diag, d_out);
   if (rc != TSLB_OK) return rc;
@@ -486,6 +562,7 @@ int tslb_diag_static(tslb_handle* h, double* out) {
     return TSLB_EINVAL;
   }
   if (!h->inited) return fail(TSLB_ESTATE, "tslb_diag_static before tslb_init");
+  if (h->split) return fail(TSLB_ESTATE, "tslb_diag_static between tslb_slab_step_faces and tslb_slab_step_interior");
   // the array belongs to the CURRENT device: it must be the one the handle's workspace is on
   cudaPointerAttributes at;
   int dev = -1;
@@ -517,6 +594,7 @@ int tslb_init_host(tslb_handle* h, const void* phi, const void* u) {
 int tslb_get_host(tslb_handle* h, void* rho, void* p, void* u, void* phi) {
   if (!h) return fail(TSLB_EINVAL, "tslb_get_host: NULL handle");
   if (!h->inited) return fail(TSLB_ESTATE, "tslb_get_host before tslb_init");
+  if (h->split) return fail(TSLB_ESTATE, "tslb_get_host between tslb_slab_step_faces and tslb_slab_step_interior");
   // derived fields go to planes 0..5 of the spare buffer, then to the host
   char* stage = h->buf[h->cur ^ 1];
   const size_t pb = size_t(h->stride) * h->es, nb = size_t(h->nodes) * h->es;

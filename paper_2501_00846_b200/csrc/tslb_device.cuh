@@ -91,6 +91,8 @@ template <typename T>
 struct DevParams {
   int nx, ny, nz;
   int bcx, bcy, bcz;          // 0 periodic, 1 wall
+  int zbeg, zend;             // output planes [zbeg, zend) of a launch of the lean pair: the whole
+                              // lattice, or one piece of a slab's split step (tslb_slab_step_*)
   long long N;
   T rho_l, rho_g, drho;       // drho = rho_l - rho_g
   T mu_g, dmu;                // mu = mu_g + phi_c dmu                      (R14)

@@ -382,8 +382,8 @@ k_stream_collide_fast(DevParams<T> P, const T* __restrict__ S, T* __restrict__ D
   int lx, ly;
   const bool mapped = M::coords(tid, lx, ly);
   const int gx = blockIdx.x * TX + lx, gy = blockIdx.y * TY + ly;
-  const int z0 = blockIdx.z * zchunk;
-  const int z1 = min(P.nz, z0 + zchunk);
+  const int z0 = P.zbeg + blockIdx.z * zchunk;
+  const int z1 = min(P.zend, z0 + zchunk);
   const int c = M::cell(lx, ly);
   const int rb = ly * TX + lx;                                  // index as a receiver (main: tid)
   const bool in_ring = mapped && gx >= -1 && gx <= P.nx && gy >= -1 && gy <= P.ny;

@@ -122,8 +122,8 @@ k_stream_collide_tma(DevParams<T> P, const __grid_constant__ TmaMaps maps, T* __
       reinterpret_cast<unsigned long long*>(tma_smem_raw + NSTAGE * sizeof(STG) + sizeof(SM));
 
   const int tid = threadIdx.x;
-  const int z0 = blockIdx.z * zchunk;
-  const int z1 = min(P.nz, z0 + zchunk);
+  const int z0 = P.zbeg + blockIdx.z * zchunk;
+  const int z1 = min(P.zend, z0 + zchunk);
   const int plane = P.nx * P.ny;
   const int gx0 = blockIdx.x * TX, gy0 = blockIdx.y * TY;
   // periodic images needed by this tile (host guarantees nx >= 2 TX, ny > TY: at most one each)

@@ -80,8 +80,8 @@ k_allen_cahn_row(DevParams<T> P, const T* __restrict__ S, const T* __restrict__ 
   const bool xhalo = warp == ROWS;                 // the extra warp: columns beside the tile
   const int gx0 = blockIdx.x * (32 * V);
   const int nact = min(32, (P.nx - gx0) / V);      // lanes of a row warp that own nodes
-  const int z0 = blockIdx.z * zchunk;
-  const int z1 = min(P.nz, z0 + zchunk);
+  const int z0 = P.zbeg + blockIdx.z * zchunk;
+  const int z1 = min(P.zend, z0 + zchunk);
   const int plane = P.nx * P.ny;
   const T* phi = S + F_PHI * P.N;
   const T c1 = T(-3.0 / 216.0), c2 = P.c2;

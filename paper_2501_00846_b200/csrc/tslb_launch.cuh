@@ -45,7 +45,7 @@ cudaError_t launch_fast(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStrea
   static bool ready[kMaxDev] = {};
   cudaError_t e = prepare(kernel, smem, ready);
   if (e != cudaSuccess) return e;
-  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.nz + zc - 1) / zc);
+  const dim3 grid((P.nx + TX - 1) / TX, (P.ny + TY - 1) / TY, (P.zend - P.zbeg + zc - 1) / zc);
   kernel<<<grid, M::NTHREADS, smem, stream>>>(P, S, D, Q, zc);
   return cudaGetLastError();
 }
@@ -136,7 +136,7 @@ cudaError_t launch_tma(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream
   static bool ready[kMaxDev] = {};
   cudaError_t e = prepare(kernel, smem, ready);
   if (e != cudaSuccess) return e;
-  const dim3 grid(P.nx / TX, (P.ny + TY - 1) / TY, (P.nz + zc - 1) / zc);
+  const dim3 grid(P.nx / TX, (P.ny + TY - 1) / TY, (P.zend - P.zbeg + zc - 1) / zc);
   kernel<<<grid, M::NTHREADS + 32, smem, stream>>>(P, tc->maps[slot], D, Q, zc);
   return cudaGetLastError();
 }
@@ -219,8 +219,9 @@ cudaError_t launch_k1_row(const DevParams<T>& P, const T* S, const T* Q, T* D, c
   int dev = 0, sms = 148;
   if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   const long long txy = (long long)((P.nx + 32 * V - 1) / (32 * V)) * ((P.ny + TY - 1) / TY);
-  const int zc = balanced_zchunk(txy, P.nz, MINB * sms);
-  const dim3 grid((P.nx + 32 * V - 1) / (32 * V), (P.ny + TY - 1) / TY, (P.nz + zc - 1) / zc);
+  const int nzr = P.zend - P.zbeg;
+  const int zc = balanced_zchunk(txy, nzr, MINB * sms);
+  const dim3 grid((P.nx + 32 * V - 1) / (32 * V), (P.ny + TY - 1) / TY, (nzr + zc - 1) / zc);
   kernel<<<grid, (TY + 3) * 32, smem, stream>>>(P, S, Q, D + F_PHI * P.N, zc);
   return cudaGetLastError();
 }
@@ -229,34 +230,42 @@ cudaError_t launch_k1_row(const DevParams<T>& P, const T* S, const T* Q, T* D, c
 enum { SEL_GENERIC = 2, SEL_K2_CPASYNC = 4, SEL_K2_TMA = 8, SEL_K1_FLUX = 16 };
 
 // One time step of the split pair: K1 (interface tracking, Eq. 20) then K2 (stream-collide-
-// moments-forces, Eq. 7-17).  Returns a cudaError_t as int.
+// moments-forces, Eq. 7-17), each over the output planes [P.zbeg, P.zend) (the whole lattice for
+// tslb_step; pieces for a slab's split step, lean pair only).  They return a cudaError_t.
+template <typename T> inline bool k1_is_tiled(const DevParams<T>& P, int flags) {
+  const bool row_ok = P.nx % RowVec<T>::V == 0;
+  return (flags & SEL_GENERIC) != 0 || ((P.bcx || P.bcy || P.bcz) && !row_ok);
+}
+
+// ---- K1 (interface tracking).  The row kernel serves periodic axes and walls (ghost positions
+// rebuild the mirrored flux from Q, phi and u); rows it cannot vectorise fall back to the
+// one-node flux kernel on all-periodic boxes and to the wall-capable kernel (normals recomputed
+// on a ring of depth 2) on boxes with walls, which hands no flux over: K2 then writes none.
 template <typename T>
-int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
-                      long long* launches, const Marker& mk, int flags, TmaCache* tc = nullptr) {
+cudaError_t launch_k1_stage(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
+                            int flags) {
+  const bool side_walls = P.bcx || P.bcy;
+  const bool row_ok = P.nx % RowVec<T>::V == 0;
+  if (k1_is_tiled(P, flags)) {
+    const bool walls = side_walls || P.bcz;
+    return walls ? launch_k1w<T, true>(P, S, D, stream) : launch_k1w<T, false>(P, S, D, stream);
+  }
+  if (row_ok && (side_walls || P.bcz || !(flags & SEL_K1_FLUX)))
+    return side_walls ? launch_k1_row<T, true>(P, S, Q, D, stream)
+                      : launch_k1_row<T, false>(P, S, Q, D, stream);
+  return launch_k1_flux<T>(P, S, Q, D, stream);
+}
+
+// ---- K2 (stream-collide-moments-forces): the lean kernel unless the wall-capable one is
+// forced; walls on z cost it two ghost planes per column (publish()), walls on x or y the
+// bounce accounting of the wall-adjacent receivers (wall_bounce, cp.async staging only)
+template <typename T>
+cudaError_t launch_k2_stage(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
+                            int flags, TmaCache* tc) {
   const bool side_walls = P.bcx || P.bcy;
   const bool forced = (flags & SEL_GENERIC) != 0;
-  const bool row_ok = P.nx % RowVec<T>::V == 0;
   cudaError_t e;
-  // ---- K1 (interface tracking).  The row kernel serves periodic axes and walls (ghost positions
-  // rebuild the mirrored flux from Q, phi and u); rows it cannot vectorise fall back to the
-  // one-node flux kernel on all-periodic boxes and to the wall-capable kernel (normals recomputed
-  // on a ring of depth 2) on boxes with walls, which hands no flux over: K2 then writes none.
-  const bool k1_tiled = forced || ((side_walls || P.bcz) && !row_ok);
-  if (k1_tiled) {
-    const bool walls = side_walls || P.bcz;
-    e = walls ? launch_k1w<T, true>(P, S, D, stream) : launch_k1w<T, false>(P, S, D, stream);
-  } else if (row_ok && (side_walls || P.bcz || !(flags & SEL_K1_FLUX))) {
-    e = side_walls ? launch_k1_row<T, true>(P, S, Q, D, stream)
-                   : launch_k1_row<T, false>(P, S, Q, D, stream);
-  } else {
-    e = launch_k1_flux<T>(P, S, Q, D, stream);
-  }
-  if (e != cudaSuccess) return int(e);
-  mk.mark(1);
-  // ---- K2 (stream-collide-moments-forces): the lean kernel unless the wall-capable one is
-  // forced; walls on z cost it two ghost planes per column (publish()), walls on x or y the
-  // bounce accounting of the wall-adjacent receivers (wall_bounce, cp.async staging only)
-  T* Qk2 = k1_tiled ? nullptr : Q;
+  T* Qk2 = k1_is_tiled(P, flags) ? nullptr : Q;
   if (forced) {
     const bool walls = side_walls || P.bcz;
     // cp.async staging pays in fp32 (0.75 vs 1.16 ms on 256^3) but not in fp64 (1.91 vs 1.83 ms)
@@ -268,8 +277,9 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
     // of 2 per 32) when the grid still fills the machine about three times over ("deep").
     constexpr int minb = sizeof(T) == 8 ? 1 : 2;
     const long long tiles = (long long)((P.nx + 31) / 32) * ((P.ny + 7) / 8);
-    const bool deep = tiles * ((P.nz + 63) / 64) >= 3LL * 148 * minb;
-    const int zc = deep ? 64 : balanced_zchunk(tiles, P.nz, 148 * minb);
+    const int nzr = P.zend - P.zbeg;
+    const bool deep = tiles * ((nzr + 63) / 64) >= 3LL * 148 * minb;
+    const int zc = deep ? 64 : balanced_zchunk(tiles, nzr, 148 * minb);
     // TMA tensor staging two planes ahead: fp64 production wherever the tile rows are full
     // (256^3: 0.79 against 0.85 ms with cp.async; 192^3, 128^3, 96^3, 64^3: +10, +8, +5, +4 % in
     // GLUPS); in fp32 (two blocks per SM) only when asked for (it loses 4 %)
@@ -288,6 +298,16 @@ int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_
       }
     }
   }
+  return e;
+}
+
+template <typename T>
+int launch_step_tiled(const DevParams<T>& P, const T* S, T* D, T* Q, cudaStream_t stream,
+                      long long* launches, const Marker& mk, int flags, TmaCache* tc = nullptr) {
+  cudaError_t e = launch_k1_stage<T>(P, S, D, Q, stream, flags);
+  if (e != cudaSuccess) return int(e);
+  mk.mark(1);
+  e = launch_k2_stage<T>(P, S, D, Q, stream, flags, tc);
   mk.mark(2);
   *launches += 2;
   return int(e);

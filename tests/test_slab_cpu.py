@@ -86,3 +86,76 @@ def test_single_rank_exchange_wraps_onto_itself():
     s = _FakeSlab(0)
     S.DistExchange(s, 0, 1, None)()
     assert s.got == (1.0, 0.0)
+
+
+# ------------------------------------------------- the overlapped schedule of SlabSolver.step
+class _StepSolver(_FakeSolver):
+    """Records the order of the calls SlabSolver.step makes; the 'faces' are a step counter."""
+
+    def __init__(self, log):
+        self.log = log
+
+    def slab_step_faces(self):
+        self.log.append("faces")
+
+    def slab_step_interior(self):
+        self.log.append("interior")
+
+    def step(self, n):
+        self.log.append("whole")
+
+
+def _step_worker(rank, world, port, q):
+    os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+    from paper_2501_00846_b200 import slab as S
+    dist.init_process_group("gloo")
+    log = []
+    sl = S.SlabSolver.__new__(S.SlabSolver)              # the schedule only: no CUDA Solver
+    sl.solver, sl.torch, sl.rank, sl.world, sl.can_split = _StepSolver(log), torch, rank, world, True
+    sl.send = [torch.zeros(3), torch.zeros(3)]
+    sl.recv = [torch.zeros(3), torch.zeros(3)]
+    sl.steps_packed, sl.seen = 0, []
+
+    def pack():
+        log.append("pack")
+        sl.steps_packed += 1
+        for f in (0, 1):
+            sl.send[f][:] = 100.0 * sl.steps_packed + 10.0 * rank + f
+
+    def unpack(lo, hi):
+        log.append("unpack")
+        sl.seen.append((float(lo[0]), float(hi[0])))
+    sl.pack, sl.unpack = pack, unpack
+    sl.exchange = S.DistExchange(sl, rank, world, dist)
+    sl.step(2, overlap=True)
+    sl.step(1, overlap=False)
+    q.put((rank, log, sl.seen))
+    dist.destroy_process_group()
+
+
+def test_overlapped_step_schedule_over_gloo():
+    """faces -> pack -> (transfers posted) -> interior -> wait + unpack, every step; each step's
+    ghosts come from the SAME step's faces of the right neighbours; overlap=False falls back to
+    whole step + exchange."""
+    world = 2
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_step_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = {r: (log, seen) for r, log, seen in (q.get(timeout=180) for _ in procs)}
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for r in range(world):
+        log, seen = res[r]
+        assert log == ["faces", "pack", "interior", "unpack"] * 2 + ["whole", "pack", "unpack"]
+        lo, hi = (r - 1) % world, (r + 1) % world
+        assert seen == [(100.0 * k + 10.0 * lo + 1, 100.0 * k + 10.0 * hi + 0) for k in (1, 2, 3)]

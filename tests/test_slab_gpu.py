@@ -12,19 +12,26 @@ from paper_2501_00846_b200 import inputs as I
 pytestmark = pytest.mark.gpu
 
 
-def _case():
-    shape = (48, 21, 70)                                         # (nz, ny, nx): ragged tiles in x, y
+def _case(nx=70):
+    shape = (48, 21, nx)                                         # (nz, ny, nx): ragged tiles in x, y
     prm = I.base_params()
     phi = I.sphere_profile(shape, (30.3, 9.1, 11.7), 8.0, 4.0, prm["bc"])      # across a slab cut
     phi += I.sphere_profile(shape, (55.2, 14.6, 36.4), 6.0, 4.0, prm["bc"])
     return dict(name="slabs", shape=shape, params=prm, phi=phi, u=I.noise_u(shape, 1e-3, 53))
 
 
-@pytest.mark.parametrize("world", [2, 4])
+@pytest.mark.parametrize("overlap", [False, True])
+@pytest.mark.parametrize("nx", [70, 64])
+@pytest.mark.parametrize("world", [2, 4, 16])
 @pytest.mark.parametrize("precision", ["f64", "f32"])
-def test_slabs_reproduce_the_single_domain(world, precision):
+def test_slabs_reproduce_the_single_domain(world, precision, nx, overlap):
+    """overlap: the step in two stages (tslb_slab_step_faces, pack, tslb_slab_step_interior,
+    unpack), the schedule that hides the exchange behind the interior sweep; it never computes
+    the ghost planes.  nx = 64 takes the TMA-staged stream-collide kernel in fp64, nx = 70 the
+    cp.async one (and, in fp32, rows the split step refuses: slab.py falls back to whole steps).
+    16 slabs of 3 planes: the two face pieces touch and there is no interior."""
     from paper_2501_00846_b200 import binding as B, slab as S
-    cfg = _case()
+    cfg = _case(nx)
     nz, ny, nx = cfg["shape"]
     one = B.Solver(nx, ny, nz, cfg["params"], precision=precision)
     one.init(cfg["phi"], cfg["u"])
@@ -35,14 +42,14 @@ def test_slabs_reproduce_the_single_domain(world, precision):
     done = 0
     for n in (1, 5, 20):
         one.step(n - done)
-        S.step_local(slabs, ex, n - done)
+        S.step_local(slabs, ex, n - done, overlap=overlap)
         done = n
         want = one.get()
         for s in slabs:
             got = s.get()
             for k, v in got.items():
                 w = want[k][..., s.z0:s.z1, :, :]
-                assert bool((v == w).all()), (world, precision, n, s.rank, k,
+                assert bool((v == w).all()), (world, precision, nx, overlap, n, s.rank, k,
                                               float((v - w).abs().max()))
     assert slabs[0].solver.launches > 0
     for s in slabs:
@@ -69,3 +76,32 @@ def test_halo_calls_reject_what_they_cannot_serve():
     with pytest.raises(B.TslbError):
         s.halo_pack(2, buf)                                      # no such face
     s.close()
+
+
+def test_split_step_state_machine():
+    """Between tslb_slab_step_faces and tslb_slab_step_interior only the halo calls are served."""
+    from paper_2501_00846_b200 import binding as B
+    cfg = _case(64)
+    nz, ny, nx = cfg["shape"]
+    s = B.Solver(nx, ny, nz, cfg["params"])
+    with pytest.raises(B.TslbError):
+        s.slab_step_faces()                                      # before tslb_init
+    s.init(cfg["phi"], cfg["u"])
+    with pytest.raises(B.TslbError):
+        s.slab_step_interior()                                   # no faces stage before it
+    s.slab_step_faces()
+    buf = s.halo_buffer()
+    s.halo_pack(0, buf)
+    s.halo_unpack(1, buf)
+    for call in (lambda: s.step(1), lambda: s.get(), lambda: s.diag(), s.slab_step_faces):
+        with pytest.raises(B.TslbError):
+            call()
+    s.slab_step_interior()
+    s.step(1)
+    s.close()
+    odd = B.Solver(70, ny, nz, cfg["params"], precision="f32")  # 70 % 4 != 0
+    c70 = _case(70)
+    odd.init(c70["phi"], c70["u"])
+    with pytest.raises(B.TslbError):
+        odd.slab_step_faces()
+    odd.close()
