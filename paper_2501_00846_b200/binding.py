@@ -24,7 +24,7 @@ SYMBOLS = ("tslb_workspace_bytes", "tslb_create", "tslb_init", "tslb_step", "tsl
            "tslb_get_state", "tslb_set_state", "tslb_init_host", "tslb_get_host", "tslb_step_timed",
            "tslb_launch_count", "tslb_diag", "tslb_diag_host", "tslb_diag_static", "tslb_fma_peak",
            "tslb_halo_bytes", "tslb_halo_pack", "tslb_halo_unpack",
-           "tslb_slab_step_faces", "tslb_slab_step_interior",
+           "tslb_slab_set_ends", "tslb_slab_step_faces", "tslb_slab_step_interior",
            "tslb_destroy", "tslb_last_error")
 
 
@@ -81,6 +81,7 @@ def load():
     lib.tslb_halo_bytes.restype = C.c_size_t
     lib.tslb_halo_pack.argtypes = [vp, C.c_int, vp]
     lib.tslb_halo_unpack.argtypes = [vp, C.c_int, vp]
+    lib.tslb_slab_set_ends.argtypes = [vp, C.c_int, C.c_int]
     lib.tslb_slab_step_faces.argtypes = [vp]
     lib.tslb_slab_step_interior.argtypes = [vp]
     lib.tslb_launch_count.argtypes = [vp]
@@ -220,6 +221,10 @@ class Solver:
 
     def halo_unpack(self, face, buf):
         self._call("tslb_halo_unpack", int(face), buf.data_ptr())
+
+    def slab_set_ends(self, ghost_low, ghost_high):
+        """Which z ends carry two ghost planes (the others are walls of the global box)."""
+        self._call("tslb_slab_set_ends", int(bool(ghost_low)), int(bool(ghost_high)))
 
     def slab_step_faces(self):
         """First stage of a slab's step: afterwards halo_pack packs the NEW face planes."""

@@ -92,6 +92,7 @@ struct tslb_handle {
   int cur;
   bool inited;
   bool split;            // between tslb_slab_step_faces and tslb_slab_step_interior
+  bool ghost[2];         // z ends that carry two ghost planes (tslb_slab_set_ends); default: both
   long long launches;
   tslb::TmaCache tma;     // tensor maps of the two state buffers (TMA-staged kernel)
 };
@@ -130,6 +131,7 @@ int tslb_create(int nx, int ny, int nz, const tslb_params* p, void* workspace, v
   h->cur = 0;
   h->inited = false;
   h->split = false;
+  h->ghost[0] = h->ghost[1] = p->bc[2] == TSLB_BC_PERIODIC;
   h->launches = 0;
   *out = h;
   return TSLB_OK;
@@ -192,12 +194,17 @@ int step_impl(tslb_handle* h, int n, const tslb::Marker& mk) {
 // computed.  Stage 0: interface update on planes [1, nz-1) (everything the owned planes' forces
 // read), stream-collide on the owned planes next to the faces, [2, 4) and [nz-4, nz-2); the
 // buffers swap, so tslb_halo_pack sees the new faces.  Stage 1: stream-collide on the interior
-// [4, nz-4).  The ghost planes are not computed at all: the exchange fills them.
+// [4, nz-4).  The ghost planes are not computed at all: the exchange fills them.  An end
+// without ghosts (a wall of the global box, tslb_slab_set_ends) has no face piece: its planes
+// belong to the interior and the wall rules of the kernels act there as in the undivided box.
 template <typename T>
 int slab_step_impl(tslb_handle* h, int stage) {
   auto P = make_dev<T>(h->nx, h->ny, h->nz, h->prm, h->stride);
   const int g = tslb::HALO_DEPTH, nz = h->nz;
-  const int lo_end = std::min(2 * g, nz - g), hi_beg = std::max(nz - 2 * g, lo_end);
+  // owned planes [own0, own1); a face piece only where the end has ghosts (a neighbour)
+  const int own0 = h->ghost[0] ? g : 0, own1 = h->ghost[1] ? nz - g : nz;
+  const int lo_end = h->ghost[0] ? std::min(own0 + g, own1) : own0;
+  const int hi_beg = h->ghost[1] ? std::max(own1 - g, lo_end) : own1;
   const T* S = reinterpret_cast<const T*>(h->buf[stage == 0 ? h->cur : h->cur ^ 1]);
   T* D = reinterpret_cast<T*>(h->buf[stage == 0 ? h->cur ^ 1 : h->cur]);
   T* Q = reinterpret_cast<T*>(h->scratch);
@@ -209,11 +216,11 @@ int slab_step_impl(tslb_handle* h, int stage) {
     h->launches += 1;
   };
   if (stage == 0) {
-    P.zbeg = 1; P.zend = nz - 1;
+    P.zbeg = h->ghost[0] ? 1 : 0; P.zend = h->ghost[1] ? nz - 1 : nz;
     e = tslb::launch_k1_stage<T>(P, S, D, Q, h->stream, h->prm.flags);
     h->launches += 1;
-    k2(g, lo_end);
-    k2(hi_beg, nz - g);
+    k2(own0, lo_end);
+    k2(hi_beg, own1);
     h->cur ^= 1;
     h->split = true;
   } else {
@@ -398,13 +405,19 @@ size_t tslb_halo_bytes(const tslb_handle* h) {
 static int halo_check(const tslb_handle* h, int face, const void* buf, const char* who) {
   if (!h || !buf || (face != 0 && face != 1)) return fail(TSLB_EINVAL, "%s: bad argument", who);
   if (!h->inited) return fail(TSLB_ESTATE, "%s before tslb_init", who);
-  if (h->prm.bc[2] != TSLB_BC_PERIODIC || h->nz < 3 * tslb::HALO_DEPTH)
-    return fail(TSLB_EINVAL, "%s: needs a periodic z axis of at least 6 planes", who);
+  if (h->nz < 3 * tslb::HALO_DEPTH)
+    return fail(TSLB_EINVAL, "%s: needs at least 6 planes along z", who);
+  if (!h->ghost[face])
+    return fail(TSLB_EINVAL, "%s: this z end has no ghost planes (a wall of the box, or "
+                "tslb_slab_set_ends said so)", who);
   if (h->prm.bc[0] != TSLB_BC_PERIODIC || h->prm.bc[1] != TSLB_BC_PERIODIC)
     return fail(TSLB_EINVAL, "%s: walls on x or y need a deeper halo than two planes (the "
                 "interface kernel recomputes the normals there)", who);
   if (h->prm.flags & (TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC))
     return fail(TSLB_EINVAL, "%s: the flux planes belong to the lean pair (flags NAIVE / GENERIC unset)", who);
+  if (h->prm.bc[2] == TSLB_BC_WALL && h->nx % (h->prm.precision == TSLB_F64 ? 2 : 4) != 0)
+    return fail(TSLB_EINVAL, "%s: with walls on z, rows that are no multiple of the 128-bit vector width "
+                "take the interface kernel that recomputes the normals (two planes of halo are not enough)", who);
   return TSLB_OK;
 }
 
@@ -425,14 +438,24 @@ int tslb_halo_unpack(tslb_handle* h, int face, const void* buf) {
 static int slab_step_check(const tslb_handle* h, const char* who) {
   if (!h) return fail(TSLB_EINVAL, "%s: NULL handle", who);
   if (!h->inited) return fail(TSLB_ESTATE, "%s before tslb_init", who);
-  if (h->prm.bc[2] != TSLB_BC_PERIODIC || h->nz < 3 * tslb::HALO_DEPTH ||
+  if (h->nz < 3 * tslb::HALO_DEPTH ||
       h->prm.bc[0] != TSLB_BC_PERIODIC || h->prm.bc[1] != TSLB_BC_PERIODIC ||
       (h->prm.flags & (TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC)))
-    return fail(TSLB_EINVAL, "%s: needs what tslb_halo_pack needs (periodic box, >= 6 planes, lean pair)", who);
+    return fail(TSLB_EINVAL, "%s: needs what tslb_halo_pack needs (periodic x and y, >= 6 planes, lean pair)", who);
   const int vec = h->prm.precision == TSLB_F64 ? 2 : 4;
   if (h->nx % vec != 0)
     return fail(TSLB_EINVAL, "%s: nx must be a multiple of %s (the row kernel of the interface update)", who,
                 vec == 2 ? "2" : "4");
+  return TSLB_OK;
+}
+
+int tslb_slab_set_ends(tslb_handle* h, int ghost_low, int ghost_high) {
+  if (!h) return fail(TSLB_EINVAL, "tslb_slab_set_ends: NULL handle");
+  if (h->split) return fail(TSLB_ESTATE, "tslb_slab_set_ends between tslb_slab_step_faces and tslb_slab_step_interior");
+  if (h->prm.bc[2] == TSLB_BC_PERIODIC && !(ghost_low && ghost_high))
+    return fail(TSLB_EINVAL, "tslb_slab_set_ends: an end without ghost planes must be a wall (bc z = TSLB_BC_WALL)");
+  h->ghost[0] = ghost_low != 0;
+  h->ghost[1] = ghost_high != 0;
   return TSLB_OK;
 }
 

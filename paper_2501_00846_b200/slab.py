@@ -1,15 +1,18 @@
-"""z-slab decomposition of a lattice that is periodic along z (the paper's
-own multi-GPU runs use Cartesian decompositions over MPI).
+"""z-slab decomposition of a lattice along z (the paper's own multi-GPU
+runs use Cartesian decompositions over MPI, "a linear decomposition along the z-axis" among them,
+PAPER.md:194-238).
 
 Orchestration only: every step of the path still runs in the kernels of libtslb.so.  Rank r of W
-owns nz / W consecutive planes and holds a Solver on nz / W + 4 planes (two ghost planes per end,
-periodic z; include/tslb.h "z-slab decomposition support").  Per time step: the step on every
-slab (in two stages, the face planes first, so that the exchange overlaps the interior sweep:
-tslb_slab_step_faces / tslb_slab_step_interior; or tslb_step(1) as a whole), and ONE exchange: each slab packs the two owned planes next to each face
-(tslb_halo_pack, 17 scalars per node), sends the low face to rank r-1 and the high face to rank r+1,
-and unpacks what it receives into its ghost planes.  The results on the owned planes are the
-single-domain results bit for bit (the kernels' per-node arithmetic does not depend on where a
-plane sits), which tests/test_slab_gpu.py checks with several slabs on ONE GPU.
+owns nz / W consecutive planes and holds a Solver on them plus two ghost planes per end that has a
+neighbour (include/tslb.h "z-slab decomposition support"): a ring when z is periodic; with walls
+on z (rising bubble, droplet train) the first and last slab end at the wall.  Per time step: the
+step on every slab (in two stages, the face planes first, so that the exchange overlaps the
+interior sweep: tslb_slab_step_faces / tslb_slab_step_interior; or tslb_step(1) as a whole), and
+ONE exchange: each slab packs the two owned planes next to each face (tslb_halo_pack, 17 scalars
+per node), sends the low face to rank r-1 and the high face to rank r+1, and unpacks what it
+receives into its ghost planes.  The results on the owned planes are the single-domain results
+bit for bit (the kernels' per-node arithmetic does not depend on where a plane sits), which
+tests/test_slab_gpu.py checks with several slabs on ONE GPU.
 
 Transport is pluggable: `LocalExchange` hands buffers over inside one process (the test, or slabs
 on the GPUs of one process); `DistExchange` uses torch.distributed point-to-point operations (NCCL
@@ -31,10 +34,18 @@ def slab_range(nz, rank, world):
     return rank * n, (rank + 1) * n
 
 
-def cut(a, z0, z1, nz):
-    """Planes [z0 - GHOST, z1 + GHOST) of a (..., nz, ny, nx) array, wrapped periodically."""
-    idx = np.arange(z0 - GHOST, z1 + GHOST) % nz
+def cut(a, z0, z1, nz, ghost=(True, True)):
+    """Planes [z0 - GHOST, z1 + GHOST) of a (..., nz, ny, nx) array, wrapped periodically; an end
+    without ghost planes (a wall of the box: ghost[end] False) is cut at the owned plane."""
+    idx = np.arange(z0 - (GHOST if ghost[0] else 0), z1 + (GHOST if ghost[1] else 0)) % nz
     return np.ascontiguousarray(np.take(a, idx, axis=-3))
+
+
+def neighbours(rank, world, periodic):
+    """(low, high) neighbour ranks of a slab; None beyond a wall of the box."""
+    if periodic:
+        return (rank - 1) % world, (rank + 1) % world
+    return (rank - 1 if rank > 0 else None), (rank + 1 if rank < world - 1 else None)
 
 
 class LocalExchange:
@@ -47,10 +58,11 @@ class LocalExchange:
         """Unpack every slab's ghosts from its neighbours' packed faces."""
         W = len(self.slabs)
         for r, s in enumerate(self.slabs):
-            lo, hi = self.slabs[(r - 1) % W], self.slabs[(r + 1) % W]
+            lo, hi = neighbours(r, W, getattr(s, "periodic", True))
             # my low ghosts = the low neighbour's high face; my high ghosts = the high
             # neighbour's low face (buffers of another slab are only read here)
-            s.unpack(lo.send[1], hi.send[0])
+            s.unpack(None if lo is None else self.slabs[lo].send[1],
+                     None if hi is None else self.slabs[hi].send[0])
 
     def __call__(self):
         for s in self.slabs:
@@ -83,25 +95,30 @@ class DistExchange:
             s.solver.synchronize()                  # host buffers: the packed faces are complete
         elif cur != own:
             cur.wait_stream(own)                    # NCCL orders its work after the CURRENT stream
-        lo, hi = (self.rank - 1) % self.world, (self.rank + 1) % self.world
-        # With two ranks both neighbours are the same peer and NCCL matches messages of a pair
-        # in posting order (no tags): the HIGH face is sent first because the peer receives its
-        # low ghosts (= its low neighbour's high face) first.
-        ops = [dist.P2POp(dist.isend, s.send[1], hi, tag=0), dist.P2POp(dist.isend, s.send[0], lo, tag=1),
-               dist.P2POp(dist.irecv, s.recv[0], lo, tag=0), dist.P2POp(dist.irecv, s.recv[1], hi, tag=1)]
-        return dist.batch_isend_irecv(ops)
+        lo, hi = neighbours(self.rank, self.world, getattr(s, "periodic", True))
+        # With two ranks on a ring both neighbours are the same peer and NCCL matches messages of
+        # a pair in posting order (no tags): the HIGH face is sent first because the peer receives
+        # its low ghosts (= its low neighbour's high face) first.  Beyond a wall of the box there
+        # is no neighbour and nothing is posted.
+        sends = ([dist.P2POp(dist.isend, s.send[1], hi, tag=0)] if hi is not None else []) + \
+                ([dist.P2POp(dist.isend, s.send[0], lo, tag=1)] if lo is not None else [])
+        recvs = ([dist.P2POp(dist.irecv, s.recv[0], lo, tag=0)] if lo is not None else []) + \
+                ([dist.P2POp(dist.irecv, s.recv[1], hi, tag=1)] if hi is not None else [])
+        return dist.batch_isend_irecv(sends + recvs)
 
     def finish(self, reqs):
         s = self.slab
         if reqs is None:                            # one rank: the slab is its own neighbour
-            s.unpack(s.send[1], s.send[0])
+            if getattr(s, "periodic", True):        # (a box with walls on z has none at all)
+                s.unpack(s.send[1], s.send[0])
             return
         for req in reqs:
             req.wait()      # NCCL: the current stream waits for the transfer; gloo: the host does
         cur, own = self._streams()
         if cur is not None and cur != own:
             own.wait_stream(cur)
-        s.unpack(s.recv[0], s.recv[1])
+        lo, hi = neighbours(self.rank, self.world, getattr(s, "periodic", True))
+        s.unpack(None if lo is None else s.recv[0], None if hi is None else s.recv[1])
 
     def __call__(self):
         self.slab.pack()
@@ -109,15 +126,21 @@ class DistExchange:
 
 
 class SlabSolver:
-    """One z slab: a Solver on the owned planes plus two ghost planes per end."""
+    """One z slab: a Solver on the owned planes plus two ghost planes per end that has a
+    neighbour.  Periodic z: a ring, every slab has both.  Walls on z (the paper's rising bubble
+    and droplet train): the first and the last slab end at the wall and carry ghosts at their inner
+    end only (tslb_slab_set_ends)."""
 
     def __init__(self, nx, ny, nz, params, rank, world, precision="f64", device="cuda:0", flags=0):
-        if tuple(params.get("bc", (0, 0, 0)))[2] != 0:
-            raise ValueError("the slab decomposition needs a periodic z axis")
+        self.periodic = tuple(params.get("bc", (0, 0, 0)))[2] == 0
         self.nz_global, self.rank, self.world = nz, rank, world
         self.z0, self.z1 = slab_range(nz, rank, world)
-        self.solver = B.Solver(nx, ny, self.z1 - self.z0 + 2 * GHOST, params, precision=precision,
-                               flags=flags, device=device)
+        lo, hi = neighbours(rank, world, self.periodic)
+        self.ghost = (lo is not None, hi is not None)
+        nzl = self.z1 - self.z0 + GHOST * (int(self.ghost[0]) + int(self.ghost[1]))
+        self.solver = B.Solver(nx, ny, nzl, params, precision=precision, flags=flags, device=device)
+        if not self.periodic:
+            self.solver.slab_set_ends(*self.ghost)
         self.torch = self.solver.torch
         self.send = [self.solver.halo_buffer(), self.solver.halo_buffer()]
         self.recv = [self.solver.halo_buffer(), self.solver.halo_buffer()]
@@ -129,16 +152,19 @@ class SlabSolver:
         """phi (nz, ny, nx), u (3, nz, ny, nx): the GLOBAL host arrays; this slab takes its part.
         The owner must run one exchange afterwards (the outermost ghost plane's force and flux
         were computed with a wrapped stencil)."""
-        self.solver.init(cut(np.asarray(phi), self.z0, self.z1, self.nz_global),
-                         cut(np.asarray(u), self.z0, self.z1, self.nz_global))
+        self.solver.init(cut(np.asarray(phi), self.z0, self.z1, self.nz_global, self.ghost),
+                         cut(np.asarray(u), self.z0, self.z1, self.nz_global, self.ghost))
 
     def pack(self):
-        self.solver.halo_pack(0, self.send[0])
-        self.solver.halo_pack(1, self.send[1])
+        for face in (0, 1):
+            if self.ghost[face]:
+                self.solver.halo_pack(face, self.send[face])
 
     def unpack(self, from_low, from_high):
-        self.solver.halo_unpack(0, from_low)
-        self.solver.halo_unpack(1, from_high)
+        if self.ghost[0] and from_low is not None:
+            self.solver.halo_unpack(0, from_low)
+        if self.ghost[1] and from_high is not None:
+            self.solver.halo_unpack(1, from_high)
 
     def step(self, n=1, overlap=True):
         """n steps, each followed by its exchange.  With `overlap` (and rows the split step
@@ -159,7 +185,9 @@ class SlabSolver:
     def get(self, want=("rho", "p", "u", "phi")):
         """The owned planes of tslb_get's fields."""
         g = self.solver.get(want)
-        return {k: v[..., GHOST:-GHOST, :, :] for k, v in g.items()}
+        a = GHOST if self.ghost[0] else 0
+        b = self.solver.nz - (GHOST if self.ghost[1] else 0)
+        return {k: v[..., a:b, :, :] for k, v in g.items()}
 
     def close(self):
         self.solver.close()

@@ -43,7 +43,8 @@ class _FakeSlab:
         pass
 
     def unpack(self, from_low, from_high):
-        self.got = (float(from_low[0]), float(from_high[0]))
+        self.got = (None if from_low is None else float(from_low[0]),
+                    None if from_high is None else float(from_high[0]))
 
 
 def _worker(rank, world, port, q):
@@ -54,6 +55,7 @@ def _worker(rank, world, port, q):
     from paper_2501_00846_b200 import slab as S
     dist.init_process_group("gloo")
     s = _FakeSlab(rank)
+    s.periodic = os.environ.get("SLAB_TEST_WALLS") != "1"
     S.DistExchange(s, rank, world, dist)()
     q.put((rank, s.got))
     dist.destroy_process_group()
@@ -78,6 +80,28 @@ def test_ring_exchange_over_gloo(world):
     for r in range(world):
         lo, hi = (r - 1) % world, (r + 1) % world
         assert res[r] == (10.0 * lo + 1, 10.0 * hi + 0), (r, res[r])
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_chain_exchange_with_walls_over_gloo(world, monkeypatch):
+    """Walls on z: no wrap between the last and the first rank; the end slabs get nothing from
+    beyond the wall."""
+    monkeypatch.setenv("SLAB_TEST_WALLS", "1")
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = dict(q.get(timeout=180) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for r in range(world):
+        want = (None if r == 0 else 10.0 * (r - 1) + 1, None if r == world - 1 else 10.0 * (r + 1))
+        assert res[r] == want, (r, res[r])
 
 
 def test_single_rank_exchange_wraps_onto_itself():
