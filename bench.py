@@ -41,8 +41,8 @@ FLOP_EXECUTED = {"f64": 603.0, "f32": 615.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per STEP (all kernels of one step) on the 256^3
 # collision workload, copied from the ncu --set full captures named beside them (not measured by
 # this run: ncu cannot run inside a timed bench)
-NCU_TRAFFIC = {"f64": (1.980335e9 + 2.102991e9 + 0.563100e9 + 0.118991e9, "profiles/r2_kernels_f64.txt"),
-               "f32": (0.977072e9 + 1.029373e9 + 0.285394e9 + 0.050653e9, "profiles/r2_kernels_f32.txt")}
+NCU_TRAFFIC = {"f64": (1.979212e9 + 2.104534e9 + 0.562511e9 + 0.118631e9, "profiles/r2_kernels_f64.txt"),
+               "f32": (0.977138e9 + 1.029165e9 + 0.285295e9 + 0.050446e9, "profiles/r2_kernels_f32.txt")}
 
 
 def parse():
