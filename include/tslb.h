@@ -132,18 +132,20 @@ int tslb_set_state(tslb_handle *h, const void *pstar, const void *u, const void 
  * The low neighbour's face-1 buffer goes into this slab's face 0 and vice versa.  The format of
  * the buffer is private to the library (same size, precision and flags on both sides).  One
  * launch each on the handle's stream, no synchronisation; after tslb_init and after every
- * tslb_step(1).  Needs >= 6 planes along z, periodic x and y, flags NAIVE / GENERIC unset (the
- * flux planes belong to the lean kernel pair), and ghost planes at that end (next paragraph).
+ * tslb_step(1).  Needs >= 6 planes along z, flags NAIVE / GENERIC unset (the flux planes belong
+ * to the lean kernel pair), ghost planes at that end (next paragraph) and, in a box with walls on
+ * any axis, nx a multiple of the 128-bit vector width (2 in fp64, 4 in fp32: other rows take an
+ * interface kernel of radius 2, for which two ghost planes are too few).
  *
  * Boxes with walls on z (the paper's rising bubble, and its droplet train, a
  * 500 x 500 x 3000 box) are cut the same way: every slab is created with bc z = TSLB_BC_WALL,
  * the first and the last one carry ghost planes at their inner end only, and
  *   tslb_slab_set_ends(h, ghost_low, ghost_high)
  * says which ends have them (default: both on a periodic z axis, none on a wall axis; an end
- * without ghosts must be a wall; nx must then be a multiple of the 128-bit vector width, 2 in
- * fp64 and 4 in fp32: other rows take an interface kernel of radius 2).  An end with ghosts
- * never applies the wall rules: what the kernels compute in the ghost planes is overwritten by
- * the exchange and the owned planes do not read beyond them.  paper_2501_00846_b200/slab.py drives it over torch.distributed. */
+ * without ghosts must be a wall).  An end with ghosts never applies the wall rules: what the
+ * kernels compute in the ghost planes is overwritten by the exchange and the owned planes do not
+ * read beyond them.  Walls on x or y need nothing special (every slab has them).
+ * paper_2501_00846_b200/slab.py drives it over torch.distributed. */
 size_t tslb_halo_bytes(const tslb_handle *h);
 int tslb_halo_pack(tslb_handle *h, int face, void *buf);
 int tslb_halo_unpack(tslb_handle *h, int face, const void *buf);

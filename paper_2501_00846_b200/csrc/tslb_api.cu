@@ -221,8 +221,10 @@ int slab_step_impl(tslb_handle* h, int stage) {
     h->launches += 1;
     k2(own0, lo_end);
     k2(hi_beg, own1);
-    h->cur ^= 1;
-    h->split = true;
+    if (e == cudaSuccess) {              // a failed launch leaves the handle at the old step
+      h->cur ^= 1;
+      h->split = true;
+    }
   } else {
     k2(lo_end, hi_beg);
     h->split = false;
@@ -410,13 +412,11 @@ static int halo_check(const tslb_handle* h, int face, const void* buf, const cha
   if (!h->ghost[face])
     return fail(TSLB_EINVAL, "%s: this z end has no ghost planes (a wall of the box, or "
                 "tslb_slab_set_ends said so)", who);
-  if (h->prm.bc[0] != TSLB_BC_PERIODIC || h->prm.bc[1] != TSLB_BC_PERIODIC)
-    return fail(TSLB_EINVAL, "%s: walls on x or y need a deeper halo than two planes (the "
-                "interface kernel recomputes the normals there)", who);
   if (h->prm.flags & (TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC))
     return fail(TSLB_EINVAL, "%s: the flux planes belong to the lean pair (flags NAIVE / GENERIC unset)", who);
-  if (h->prm.bc[2] == TSLB_BC_WALL && h->nx % (h->prm.precision == TSLB_F64 ? 2 : 4) != 0)
-    return fail(TSLB_EINVAL, "%s: with walls on z, rows that are no multiple of the 128-bit vector width "
+  const bool walls = h->prm.bc[0] == TSLB_BC_WALL || h->prm.bc[1] == TSLB_BC_WALL || h->prm.bc[2] == TSLB_BC_WALL;
+  if (walls && h->nx % (h->prm.precision == TSLB_F64 ? 2 : 4) != 0)
+    return fail(TSLB_EINVAL, "%s: in a box with walls, rows that are no multiple of the 128-bit vector width "
                 "take the interface kernel that recomputes the normals (two planes of halo are not enough)", who);
   return TSLB_OK;
 }
@@ -438,10 +438,8 @@ int tslb_halo_unpack(tslb_handle* h, int face, const void* buf) {
 static int slab_step_check(const tslb_handle* h, const char* who) {
   if (!h) return fail(TSLB_EINVAL, "%s: NULL handle", who);
   if (!h->inited) return fail(TSLB_ESTATE, "%s before tslb_init", who);
-  if (h->nz < 3 * tslb::HALO_DEPTH ||
-      h->prm.bc[0] != TSLB_BC_PERIODIC || h->prm.bc[1] != TSLB_BC_PERIODIC ||
-      (h->prm.flags & (TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC)))
-    return fail(TSLB_EINVAL, "%s: needs what tslb_halo_pack needs (periodic x and y, >= 6 planes, lean pair)", who);
+  if (h->nz < 3 * tslb::HALO_DEPTH || (h->prm.flags & (TSLB_FLAG_NAIVE | TSLB_FLAG_GENERIC)))
+    return fail(TSLB_EINVAL, "%s: needs what tslb_halo_pack needs (>= 6 planes along z, lean pair)", who);
   const int vec = h->prm.precision == TSLB_F64 ? 2 : 4;
   if (h->nx % vec != 0)
     return fail(TSLB_EINVAL, "%s: nx must be a multiple of %s (the row kernel of the interface update)", who,

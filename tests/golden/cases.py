@@ -33,7 +33,7 @@ CASES = {
                      [1, 10, 100, 1000, 2000, 3000, 4000, 5000]),
     "emulsion192": (lambda: I.emulsion_sweep(n=192, n_drops=25), [1, 10, 100, 500, 1000]),
     # ---- configs[4]: emulsion at 384^3 (the oracle needs ~40 GB there; 512^3 does not fit)
-    "emulsion384": (lambda: I.emulsion_sweep(n=384), [1, 5, 10, 20, 50]),
+    "emulsion384": (lambda: I.emulsion_sweep(n=384), [1, 5, 10, 20, 50, 100, 150, 200, 250]),
     # ---- NEXT-2: off-axis collision, impact parameter 0.4, at 128^3
     "offaxis128": (lambda: I.off_axis_collision(n=128, impact=0.4), [1, 10, 100, 300]),
     # ---- NEXT-2, second workload: a train of 5 droplets falling onto the bottom

@@ -28,6 +28,9 @@ CASES = {
                        [1000, 2000, 20000]),          # 20000 = configs[2]'s own step count
     "collision64": (lambda: I.head_on_collision(n=64, radius=6.0, half_sep=10.0), [1000, 1500]),
     "offaxis64": (lambda: I.off_axis_collision(n=64, impact=0.4), [600, 1200]),
+    # droplet train onto the bottom wall (NEXT-2, R20b): during the first spreading (contact near
+    # step 190), after the second impact (~580), and the film long after the third
+    "train48x48x96": (lambda: I.droplet_train(nx=48, ny=48, nz=96, n_drops=3), [250, 700, 3000]),
 }
 
 
