@@ -40,4 +40,7 @@ CASES = {
     # wall (walls in z, gravity on the liquid, R20b); first contact near step 256, then every 512
     "train64x64x192": (lambda: I.droplet_train(nx=64, ny=64, nz=192),
                        [1, 10, 100, 300, 600, 1000, 1500]),
+    # ... and at the grid bench.py --workload train times (first contact near step 512)
+    "train128x128x768": (lambda: I.droplet_train(nx=128, ny=128, nz=768),
+                         [1, 10, 100, 300, 500, 600, 700, 800, 900, 1000, 1100, 1200]),
 }
