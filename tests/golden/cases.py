@@ -42,5 +42,5 @@ CASES = {
                        [1, 10, 100, 300, 600, 1000, 1500]),
     # ... and at the grid bench.py --workload train times (first contact near step 512)
     "train128x128x768": (lambda: I.droplet_train(nx=128, ny=128, nz=768),
-                         [1, 10, 100, 300, 500, 600, 700, 800, 900, 1000, 1100, 1200]),
+                         [1, 10, 100, 300, 500, 600, 700]),
 }
